@@ -1,0 +1,148 @@
+/* ternary_sa.h — C ABI of the B200-native parallel simulated-annealing library for ternary
+ * (Low/Medium/High) discrete logic regulatory networks.
+ *
+ * Method: arxiv 2506.19866, "GPU-accelerated modeling of biological regulatory networks"
+ * (PAPER.md under /root/reference): Table 1 is the chain step, §2.1
+ * the node update, §2.3 the objective.  The model is the
+ * simplified "config model" that BASELINE.json pins (DESIGN.md §1/§3).
+ *
+ * All pointers in this header are HOST pointers unless a comment says "device".  The caller owns
+ * every input array; the library copies what it needs during the call and keeps no caller
+ * pointer.  Outputs go to caller-allocated host buffers of the documented size.
+ *
+ * Every function that returns int returns SA_OK (0) or a negative code; sa_last_error() then
+ * holds a message (thread-local).  Nothing throws or exits across this boundary.  A handle is not
+ * thread-safe.  There is no CPU fallback: without a CUDA device sa_create fails with SA_ECUDA.
+ */
+#ifndef TERNARY_SA_H
+#define TERNARY_SA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SA_OK      0
+#define SA_EINVAL -1   /* bad sizes / values / ordering / NULL pointer */
+#define SA_ENOMEM -2   /* host or device allocation failed */
+#define SA_ECUDA  -3   /* CUDA runtime error; text in sa_last_error() */
+
+#define SA_UNOBSERVED 255u
+
+typedef struct sa_handle sa_handle;              /* opaque, owned by the library */
+
+/* Candidate structure: nodes and directed candidate edges whose weight may become 0
+ * (Fig.1 caption :176).  No self-loops, no duplicate (src,dst). */
+typedef struct {
+  int32_t n_nodes, n_edges;                      /* N, E */
+  const int32_t *edge_src, *edge_dst;            /* [E], in [0,N) */
+  int32_t n_pairs;                               /* number of (t_lo,t_hi) pairs, 6 in all configs; <= 16 */
+  const int8_t *th_lo, *th_hi;                   /* [n_pairs], th_lo[q] < th_hi[q] */
+} sa_network;
+
+/* Experimental conditions and discretised time-course observations (the
+ * reference matrix R; here one [n_obs][N] block per condition, 255 = entity not measured). */
+typedef struct {
+  int32_t n_cond, n_steps, n_obs;                /* K, T, n_obs */
+  const int32_t *obs_times;                      /* [n_obs], strictly increasing, in [1,T] */
+  const uint8_t *init_state;                     /* [K][N] in {0,1,2}: state at t = 0 (never scored) */
+  const uint8_t *clamp;                          /* [K][N] 0/1: a clamped node keeps init_state for all t */
+  const uint8_t *obs;                            /* [K][n_obs][N] in {0,1,2} or SA_UNOBSERVED; may be NULL
+                                                    for sa_simulate only */
+} sa_observations;
+
+/* Annealing schedule (temperature levels, iterations per level). */
+typedef struct {
+  int32_t  n_chains;                             /* R chains held by this handle */
+  uint64_t seed;                                 /* Philox key */
+  int32_t  n_levels, steps_per_level, dmax;      /* L, S_l, D */
+  const uint32_t *accept;                        /* [L][D]: floor(2^32 * exp(-d/T_l)), d = 1..D */
+  uint32_t chain_id_base;                        /* global id of chain 0 (chain-range partition over
+                                                    GPUs, reading 25); usually 0 */
+} sa_schedule;
+
+/* Parameter vector layout everywhere in this ABI: int8 params[E+N];
+ *   params[e]     = weight of edge e (caller's edge order), in {-1,0,+1};
+ *   params[E + i] = threshold-pair index of node i, in [0, n_pairs). */
+
+/* Build the device-resident problem, allocate the chain store (SoA int8 in HBM), initialise
+ * every chain from Philox domain 1 and evaluate its fitness.
+ * Validation (SA_EINVAL): counts > 0, endpoints in range, no self-loop / duplicate edge,
+ * th_lo < th_hi, states in {0,1,2}, obs in {0,1,2,255}, obs_times strictly increasing in [1,T],
+ * accumulator range: 128 + s - th_lo[q] and 128 + s - th_hi[q] - 1 in [0,255] for all |s| <=
+ * 2*max_in_degree (in-degree <= 62 with thresholds in [-3,3]).  On failure *out = NULL. */
+int sa_create(const sa_network *net, const sa_observations *obs, const sa_schedule *sched, sa_handle **out);
+
+/* Advance every chain by `steps` SA steps (Table 1 inner loop :130-149; SURVEY.md
+ * §8(c)-3): propose, simulate all K conditions for T steps, score, accept/reject, commit.
+ * Asynchronous on the handle's stream.  The global step counter persists across calls;
+ * level(g) = min(g / steps_per_level, L-1).  sa_run(a); sa_run(b) == sa_run(a+b). */
+int sa_run(sa_handle *h, int64_t steps);
+
+/* Chain with the smallest best fitness (ties: smallest chain index).  Any output may be NULL.
+ * params receives E+N bytes.  Synchronises the stream.  (min over threads.) */
+int sa_best(sa_handle *h, uint32_t *fitness, int32_t *chain, int8_t *params);
+
+void sa_destroy(sa_handle *h);                   /* NULL is a no-op */
+
+/* ---- diagnostics (parity and tests) ---- */
+
+/* Fitness (PAPER.md:104-111 as the 0/1 mismatch count) of n given parameter
+ * sets, params [n][E+N] -> fitness [n].  Same simulate/score code as sa_run. */
+int sa_eval(sa_handle *h, const int8_t *params, int64_t n, uint32_t *fitness);
+
+/* Simulate one parameter set and return the states at the observation times,
+ * states [K][n_obs][N] in {0,1,2} (Simulate() generates pseudo-experimental time
+ * series).  Needs no handle; obs->obs is ignored and may be NULL. */
+int sa_simulate(const sa_network *net, const sa_observations *obs, const int8_t *params, uint8_t *states);
+
+/* One chain's current and best vectors ([E+N] each) and fitnesses.  Any output may be NULL. */
+int sa_get_chain(sa_handle *h, int32_t chain, int8_t *cur, uint32_t *cur_fit, int8_t *best, uint32_t *best_fit);
+
+/* All chains' current / best fitness, [R] each.  Either may be NULL. */
+int sa_get_fitness(sa_handle *h, uint32_t *cur_fit, uint32_t *best_fit);
+
+/* Trace the next sa_run calls for `n` chains (local indices): one u64 record per traced chain
+ * per step, up to max_steps steps counted from the step counter at the time of this call.
+ * Record: bits 0-31 delta_cand, 32-55 parameter index p, 56-59 new value code (weight+1 or pair
+ * index), bit 60 accepted, bit 61 new best.  n = 0 switches tracing off. */
+int sa_set_trace(sa_handle *h, const int32_t *chains, int32_t n, int64_t max_steps);
+
+/* records [n][max_steps] (row order = order given to sa_set_trace); steps not yet run are 0. */
+int sa_get_trace(sa_handle *h, uint64_t *records);
+
+/* Host helper, double precision: T_l = t0*(t_end/t0)^(l/(L-1)), T_0 = t0 if
+ * L == 1; out[l*D + d-1] = floor(2^32 * exp(-d/T_l)) clamped to 2^32-1. */
+int sa_geometric_table(double t0, double t_end, int32_t n_levels, int32_t dmax, uint32_t *out);
+
+/* Which kernel family a handle uses and how it was launched (for bench.py / DESIGN.md):
+ * info[0] = kernel variant id, [1] = threads per CTA, [2] = chains per CTA, [3] = dynamic shared
+ * memory bytes per CTA, [4] = CTAs in the sa_run grid, [5] = padded edge slots, [6] = SM count,
+ * [7] = kernels launched so far by this handle. */
+int sa_get_info(sa_handle *h, int64_t info[8]);
+
+/* ---- plumbing ---- */
+
+/* CUDA stream (cudaStream_t as void*) the handle's kernels and copies run on; default stream 0. */
+int sa_set_stream(sa_handle *h, void *cuda_stream);
+
+/* Process-wide device allocator hooks (e.g. PyTorch's caching allocator); NULL, NULL restores
+ * cudaMalloc / cudaFree.  alloc returns a DEVICE pointer or NULL.  Set before sa_create. */
+typedef void *(*sa_alloc_fn)(size_t bytes, void *cuda_stream);
+typedef void (*sa_free_fn)(void *device_ptr);
+int sa_set_allocator(sa_alloc_fn alloc, sa_free_fn release);
+
+/* Roofline denominator, measured: issue rates of independent integer instruction streams on
+ * the current device.  out[0] = IADD3, [1] = LOP3, [2] = IMAD, [3] = mixed IADD3+IMAD,
+ * in warp-instructions per second (whole GPU); out[4] = SM count, out[5] = SM clock in Hz as
+ * observed through clock64 over the run.  (SURVEY.md §8(d) "Which roofline".) */
+int sa_int32_peak(double out[6]);
+
+const char *sa_last_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TERNARY_SA_H */

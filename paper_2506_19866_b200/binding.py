@@ -1,0 +1,234 @@
+"""Thin ctypes binding of libternary_sa.so — same names as include/ternary_sa.h, argument
+marshalling only.  Every step of the path runs in the library's CUDA kernels; there is no CPU
+fallback: importing this module raises if the library is missing.
+
+PyTorch is plumbing: ``use_torch_plumbing()`` plugs its caching allocator in as the library's
+device allocator and ``sa_create`` binds the handle to torch's current CUDA stream.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libternary_sa.so")
+
+SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
+EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
+           "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
+           "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error")
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2506_19866_b200.build` "
+                      "(or __graft_entry__.build()); there is no CPU fallback")
+_lib = C.CDLL(LIB_PATH)
+
+
+class SaError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = _lib.sa_last_error()
+        super().__init__(f"{where} failed ({code}): {msg.decode() if msg else ''}")
+
+
+class _Network(C.Structure):
+    _fields_ = [("n_nodes", C.c_int32), ("n_edges", C.c_int32), ("edge_src", C.c_void_p), ("edge_dst", C.c_void_p),
+                ("n_pairs", C.c_int32), ("th_lo", C.c_void_p), ("th_hi", C.c_void_p)]
+
+
+class _Observations(C.Structure):
+    _fields_ = [("n_cond", C.c_int32), ("n_steps", C.c_int32), ("n_obs", C.c_int32), ("obs_times", C.c_void_p),
+                ("init_state", C.c_void_p), ("clamp", C.c_void_p), ("obs", C.c_void_p)]
+
+
+class _Schedule(C.Structure):
+    _fields_ = [("n_chains", C.c_int32), ("seed", C.c_uint64), ("n_levels", C.c_int32),
+                ("steps_per_level", C.c_int32), ("dmax", C.c_int32), ("accept", C.c_void_p),
+                ("chain_id_base", C.c_uint32)]
+
+
+ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
+FREE_FN = C.CFUNCTYPE(None, C.c_void_p)
+
+_lib.sa_last_error.restype = C.c_char_p
+_lib.sa_create.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.POINTER(_Schedule), C.POINTER(C.c_void_p)]
+_lib.sa_run.argtypes = [C.c_void_p, C.c_int64]
+_lib.sa_best.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sa_destroy.argtypes = [C.c_void_p]
+_lib.sa_destroy.restype = None
+_lib.sa_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+_lib.sa_simulate.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c_void_p, C.c_void_p]
+_lib.sa_get_chain.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sa_get_fitness.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sa_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64]
+_lib.sa_get_trace.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sa_geometric_table.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_void_p]
+_lib.sa_get_info.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sa_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sa_set_allocator.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sa_int32_peak.argtypes = [C.c_void_p]
+
+
+def _check(rc: int, where: str):
+    if rc != SA_OK:
+        raise SaError(rc, where)
+
+
+def _arr(a, dtype) -> np.ndarray:
+    return np.ascontiguousarray(a, dtype=dtype)
+
+
+def _marshal_problem(prob, need_obs: bool = True):
+    keep = {
+        "src": _arr(prob.edge_src, np.int32), "dst": _arr(prob.edge_dst, np.int32),
+        "lo": _arr(prob.th_lo, np.int8), "hi": _arr(prob.th_hi, np.int8),
+        "times": _arr(prob.obs_times, np.int32), "init": _arr(prob.init_state, np.uint8),
+        "clamp": _arr(prob.clamp, np.uint8),
+    }
+    net = _Network(prob.n_nodes, prob.n_edges, keep["src"].ctypes.data, keep["dst"].ctypes.data,
+                   keep["lo"].shape[0], keep["lo"].ctypes.data, keep["hi"].ctypes.data)
+    obs_ptr = None
+    if need_obs:
+        keep["obs"] = _arr(prob.obs, np.uint8)
+        obs_ptr = keep["obs"].ctypes.data
+    obs = _Observations(prob.n_cond, prob.n_steps, keep["times"].shape[0], keep["times"].ctypes.data,
+                        keep["init"].ctypes.data, keep["clamp"].ctypes.data, obs_ptr)
+    return net, obs, keep
+
+
+# ------------------------------------------------------------------------------- plumbing
+_hooks = None
+
+
+def use_torch_plumbing() -> None:
+    """Device memory from PyTorch's CUDA caching allocator (process-wide hook)."""
+    global _hooks
+    if _hooks is not None:
+        return
+    import torch
+
+    def _alloc(nbytes, stream):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes), stream=int(stream or 0))
+        except Exception:
+            return None
+
+    def _free(ptr):
+        try:
+            torch.cuda.caching_allocator_delete(int(ptr))
+        except Exception:
+            pass
+
+    _hooks = (ALLOC_FN(_alloc), FREE_FN(_free))
+    _check(_lib.sa_set_allocator(C.cast(_hooks[0], C.c_void_p), C.cast(_hooks[1], C.c_void_p)), "sa_set_allocator")
+
+
+def sa_set_allocator_default() -> None:
+    global _hooks
+    _check(_lib.sa_set_allocator(None, None), "sa_set_allocator")
+    _hooks = None
+
+
+# ------------------------------------------------------------------------------- the ABI
+def sa_geometric_table(t0: float, t_end: float, n_levels: int, dmax: int) -> np.ndarray:
+    out = np.zeros((n_levels, dmax), dtype=np.uint32)
+    _check(_lib.sa_geometric_table(t0, t_end, n_levels, dmax, out.ctypes.data), "sa_geometric_table")
+    return out
+
+
+def sa_create(prob, sched, stream: Optional[int] = None) -> int:
+    """prob / sched: objects with the fields of problems.Problem / problems.Schedule.  Returns the handle."""
+    net, obs, keep = _marshal_problem(prob)
+    table = _arr(sched.accept, np.uint32)
+    sc = _Schedule(sched.n_chains, sched.seed, sched.n_levels, sched.steps_per_level, sched.dmax,
+                   table.ctypes.data, getattr(sched, "chain_id_base", 0))
+    h = C.c_void_p()
+    _check(_lib.sa_create(C.byref(net), C.byref(obs), C.byref(sc), C.byref(h)), "sa_create")
+    if stream is None and _hooks is not None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    if stream:
+        _check(_lib.sa_set_stream(h, C.c_void_p(stream)), "sa_set_stream")
+    return h.value
+
+
+def sa_set_stream(h: int, stream: int) -> None:
+    _check(_lib.sa_set_stream(h, C.c_void_p(stream)), "sa_set_stream")
+
+
+def sa_run(h: int, steps: int) -> None:
+    _check(_lib.sa_run(h, steps), "sa_run")
+
+
+def sa_best(h: int, n_params: int):
+    fit, chain = C.c_uint32(), C.c_int32()
+    params = np.zeros(n_params, dtype=np.int8)
+    _check(_lib.sa_best(h, C.byref(fit), C.byref(chain), params.ctypes.data), "sa_best")
+    return fit.value, chain.value, params
+
+
+def sa_destroy(h: int) -> None:
+    _lib.sa_destroy(h)
+
+
+def sa_eval(h: int, params) -> np.ndarray:
+    x = _arr(params, np.int8)
+    x = x.reshape(-1, x.shape[-1])
+    out = np.zeros(x.shape[0], dtype=np.uint32)
+    _check(_lib.sa_eval(h, x.ctypes.data, x.shape[0], out.ctypes.data), "sa_eval")
+    return out
+
+
+def sa_simulate(prob, params) -> np.ndarray:
+    net, obs, keep = _marshal_problem(prob, need_obs=False)
+    x = _arr(params, np.int8)
+    out = np.zeros((prob.n_cond, keep["times"].shape[0], prob.n_nodes), dtype=np.uint8)
+    _check(_lib.sa_simulate(C.byref(net), C.byref(obs), x.ctypes.data, out.ctypes.data), "sa_simulate")
+    return out
+
+
+def sa_get_chain(h: int, chain: int, n_params: int):
+    cur = np.zeros(n_params, dtype=np.int8)
+    best = np.zeros(n_params, dtype=np.int8)
+    fc, fb = C.c_uint32(), C.c_uint32()
+    _check(_lib.sa_get_chain(h, chain, cur.ctypes.data, C.byref(fc), best.ctypes.data, C.byref(fb)), "sa_get_chain")
+    return cur, fc.value, best, fb.value
+
+
+def sa_get_fitness(h: int, n_chains: int):
+    cur = np.zeros(n_chains, dtype=np.uint32)
+    best = np.zeros(n_chains, dtype=np.uint32)
+    _check(_lib.sa_get_fitness(h, cur.ctypes.data, best.ctypes.data), "sa_get_fitness")
+    return cur, best
+
+
+def sa_set_trace(h: int, chains: Sequence[int], max_steps: int) -> None:
+    c = _arr(list(chains), np.int32)
+    _check(_lib.sa_set_trace(h, c.ctypes.data if c.size else None, int(c.size), max_steps), "sa_set_trace")
+
+
+def sa_get_trace(h: int, n_chains: int, max_steps: int) -> np.ndarray:
+    out = np.zeros((n_chains, max_steps), dtype=np.uint64)
+    _check(_lib.sa_get_trace(h, out.ctypes.data), "sa_get_trace")
+    return out
+
+
+def sa_get_info(h: int) -> dict:
+    info = np.zeros(8, dtype=np.int64)
+    _check(_lib.sa_get_info(h, info.ctypes.data), "sa_get_info")
+    keys = ("variant", "threads_per_cta", "chains_per_cta", "smem_bytes", "grid", "edge_slots", "sm_count", "launches")
+    return dict(zip(keys, (int(v) for v in info)))
+
+
+def sa_int32_peak() -> dict:
+    out = np.zeros(6, dtype=np.float64)
+    _check(_lib.sa_int32_peak(out.ctypes.data), "sa_int32_peak")
+    return {"iadd3": out[0], "lop3": out[1], "imad": out[2], "mixed": out[3], "sm_count": int(out[4]), "sm_hz": out[5]}
+
+
+def sa_last_error() -> str:
+    msg = _lib.sa_last_error()
+    return msg.decode() if msg else ""

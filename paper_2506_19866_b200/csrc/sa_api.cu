@@ -1,0 +1,384 @@
+// C ABI of libternary_sa.so (include/ternary_sa.h): argument checking, device memory, launches.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <memory>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/ternary_sa.h"
+#include "sa_common.h"
+#include "sa_kernels.h"
+#include "sa_plan.h"
+
+namespace {
+
+thread_local std::string g_err;
+sa_alloc_fn g_alloc = nullptr;
+sa_free_fn g_free = nullptr;
+
+int set_err(int code, const std::string& msg) {
+  g_err = msg;
+  return code;
+}
+
+int cuda_err(cudaError_t e, const char* what) {
+  return set_err(SA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+}
+
+#define TSA_CUDA(call)                                   \
+  do {                                                   \
+    cudaError_t e__ = (call);                            \
+    if (e__ != cudaSuccess) return cuda_err(e__, #call); \
+  } while (0)
+
+// Device buffers owned by a handle; released through the hooks they were allocated with.
+struct DevPool {
+  std::vector<void*> ptrs;
+  sa_free_fn release = nullptr;
+  bool hooked = false;
+  ~DevPool() { clear(); }
+  void clear() {
+    for (void* p : ptrs) {
+      if (!p) continue;
+      if (hooked) release(p); else cudaFree(p);
+    }
+    ptrs.clear();
+  }
+  void* alloc(size_t bytes, cudaStream_t st) {
+    if (bytes == 0) bytes = 16;
+    void* p = nullptr;
+    if (ptrs.empty()) { hooked = (g_alloc && g_free); release = g_free; }
+    if (hooked) p = g_alloc(bytes, (void*)st);
+    else if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); p = nullptr; }
+    if (p) ptrs.push_back(p);
+    return p;
+  }
+  template <typename T>
+  int upload(const std::vector<T>& v, const T** out, cudaStream_t st) {
+    T* d = (T*)alloc(v.size() * sizeof(T), st);
+    if (!d) return set_err(SA_ENOMEM, "device allocation failed");
+    if (!v.empty()) TSA_CUDA(cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st));
+    *out = d;
+    return SA_OK;
+  }
+};
+
+int upload_problem(const tsa::Plan& pl, DevPool& pool, tsa::DevProblem* P, cudaStream_t st) {
+  tsa::DevProblem& d = *P;
+  std::memset(&d, 0, sizeof(d));
+  d.N = pl.N; d.E = pl.E; d.P = pl.P; d.K = pl.K; d.T = pl.T; d.n_obs = pl.n_obs; d.n_pairs = pl.n_pairs;
+  d.CG = pl.CG; d.n_chunks = pl.n_chunks; d.n_pass = pl.n_pass; d.Epad = pl.Epad; d.EpadA = pl.EpadA;
+  d.NpadA = pl.NpadA; d.state_words = pl.state_words;
+  std::memcpy(d.tha, pl.tha, sizeof(d.tha));
+  std::memcpy(d.thb, pl.thb, sizeof(d.thb));
+  int rc;
+  if ((rc = pool.upload(pl.pass_base, &d.pass_base, st))) return rc;
+  if ((rc = pool.upload(pl.pass_deg, &d.pass_deg, st))) return rc;
+  if ((rc = pool.upload(pl.slot_off, &d.slot_off, st))) return rc;
+  if ((rc = pool.upload(pl.slot_of_param, &d.slot_of_param, st))) return rc;
+  if ((rc = pool.upload(pl.row_of_node, &d.row_of_node, st))) return rc;
+  if ((rc = pool.upload(pl.node_of_row, &d.node_of_row, st))) return rc;
+  if ((rc = pool.upload(pl.initw, &d.initw, st))) return rc;
+  if ((rc = pool.upload(pl.clampm, &d.clampm, st))) return rc;
+  if ((rc = pool.upload(pl.obsw, &d.obsw, st))) return rc;
+  if ((rc = pool.upload(pl.obsm, &d.obsm, st))) return rc;
+  if ((rc = pool.upload(pl.obs_idx_of_t, &d.obs_idx_of_t, st))) return rc;
+  return SA_OK;
+}
+
+int pick_threads(const tsa::DevProblem& P, int64_t n_ctas, int sm_count) {
+  if (const char* env = std::getenv("TSA_TEAM_WARPS")) {
+    int w = std::atoi(env);
+    if (w >= 1 && w <= 32) return 32 * w;
+  }
+  // aim at ~32 resident warps per SM: CTAs per SM are bounded by shared memory, the 32-CTA limit
+  // and the grid itself; the rest comes from warps per chain (at most one per pass, at most 8)
+  const size_t sb = tsa::smem_bytes(P) + 1024;
+  int64_t per_sm = std::min<int64_t>(32, (int64_t)(227 * 1024 / sb));
+  per_sm = std::max<int64_t>(1, std::min<int64_t>(per_sm, (n_ctas + sm_count - 1) / sm_count));
+  int warps = (int)std::max<int64_t>(1, 32 / per_sm);
+  warps = std::min(warps, std::min(P.n_pass, 8));
+  return 32 * warps;
+}
+
+}  // namespace
+
+struct sa_handle {
+  tsa::Plan plan;
+  tsa::DevProblem P;
+  tsa::DevChains C;
+  tsa::DevSched S;
+  tsa::DevTrace Tr;
+  DevPool pool;         // problem + chain store
+  DevPool trace_pool;   // trace buffers (re-armed by sa_set_trace)
+  cudaStream_t stream = 0;
+  uint64_t g = 0;       // global step counter
+  int threads = 32;
+  int sm_count = 148;
+  int64_t launches = 0;
+  int32_t n_traced = 0;
+  int64_t trace_steps = 0;
+};
+
+extern "C" {
+
+const char* sa_last_error(void) { return g_err.c_str(); }
+
+int sa_set_allocator(sa_alloc_fn alloc, sa_free_fn release) {
+  if ((alloc == nullptr) != (release == nullptr)) return set_err(SA_EINVAL, "give both hooks or neither");
+  g_alloc = alloc;
+  g_free = release;
+  return SA_OK;
+}
+
+int sa_geometric_table(double t0, double t_end, int32_t L, int32_t D, uint32_t* out) {
+  if (!out || L <= 0 || D <= 0 || !(t0 > 0.0) || !(t_end > 0.0)) return set_err(SA_EINVAL, "bad table arguments");
+  for (int l = 0; l < L; ++l) {
+    const double temp = (L == 1) ? t0 : t0 * std::pow(t_end / t0, (double)l / (double)(L - 1));
+    for (int d = 1; d <= D; ++d) {
+      const double v = std::floor(4294967296.0 * std::exp(-(double)d / temp));
+      out[(size_t)l * D + (d - 1)] = v >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)v;
+    }
+  }
+  return SA_OK;
+}
+
+int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedule* sched, sa_handle** out) {
+  if (!out) return set_err(SA_EINVAL, "out is NULL");
+  *out = nullptr;
+  if (!net || !obs || !sched) return set_err(SA_EINVAL, "null argument");
+  if (sched->n_chains <= 0 || sched->n_levels <= 0 || sched->steps_per_level <= 0 || sched->dmax <= 0 || !sched->accept)
+    return set_err(SA_EINVAL, "bad schedule");
+  std::unique_ptr<sa_handle> h(new (std::nothrow) sa_handle());
+  if (!h) return set_err(SA_ENOMEM, "host allocation failed");
+  std::string err;
+  int rc = tsa::build_plan(net, obs, true, &h->plan, &err);
+  if (rc != SA_OK) return set_err(rc, err);
+
+  int dev = 0;
+  TSA_CUDA(cudaGetDevice(&dev));
+  TSA_CUDA(cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
+  cudaStream_t st = h->stream;
+  if ((rc = upload_problem(h->plan, h->pool, &h->P, st))) return rc;
+
+  const int R = sched->n_chains;
+  tsa::DevChains& C = h->C;
+  C.R = R;
+  C.cur_w = (int8_t*)h->pool.alloc((size_t)R * h->P.EpadA, st);
+  C.best_w = (int8_t*)h->pool.alloc((size_t)R * h->P.EpadA, st);
+  C.cur_th = (int8_t*)h->pool.alloc((size_t)R * h->P.NpadA, st);
+  C.best_th = (int8_t*)h->pool.alloc((size_t)R * h->P.NpadA, st);
+  C.fit_cur = (uint32_t*)h->pool.alloc((size_t)R * 4, st);
+  C.fit_best = (uint32_t*)h->pool.alloc((size_t)R * 4, st);
+  if (!C.cur_w || !C.best_w || !C.cur_th || !C.best_th || !C.fit_cur || !C.fit_best)
+    return set_err(SA_ENOMEM, "device allocation failed (chain store)");
+
+  tsa::DevSched& S = h->S;
+  S.key0 = (uint32_t)sched->seed; S.key1 = (uint32_t)(sched->seed >> 32);
+  S.chain_id_base = sched->chain_id_base;
+  S.n_levels = sched->n_levels; S.dmax = sched->dmax; S.steps_per_level = sched->steps_per_level;
+  {
+    std::vector<uint32_t> tab(sched->accept, sched->accept + (size_t)sched->n_levels * sched->dmax);
+    if ((rc = h->pool.upload(tab, &S.accept, st))) return rc;
+  }
+  std::memset(&h->Tr, 0, sizeof(h->Tr));
+
+  const size_t sb = tsa::smem_bytes(h->P);
+  if (sb > 227 * 1024) return set_err(SA_EINVAL, "chain state does not fit shared memory (N, E too large for this kernel family)");
+  h->threads = pick_threads(h->P, R, h->sm_count);
+  TSA_CUDA(tsa::launch_init(h->P, h->C, h->S, h->threads, st));
+  ++h->launches;
+  TSA_CUDA(cudaStreamSynchronize(st));   // host vectors used by the async uploads die with this frame
+  *out = h.release();
+  return SA_OK;
+}
+
+void sa_destroy(sa_handle* h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->stream);
+  delete h;
+}
+
+int sa_set_stream(sa_handle* h, void* cuda_stream) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  h->stream = (cudaStream_t)cuda_stream;
+  return SA_OK;
+}
+
+int sa_run(sa_handle* h, int64_t steps) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  if (steps < 0) return set_err(SA_EINVAL, "steps < 0");
+  if (steps == 0) return SA_OK;
+  TSA_CUDA(tsa::launch_run(h->P, h->C, h->S, h->Tr, h->g, steps, h->threads, h->stream));
+  ++h->launches;
+  h->g += (uint64_t)steps;
+  return SA_OK;
+}
+
+int sa_get_fitness(sa_handle* h, uint32_t* cur_fit, uint32_t* best_fit) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  const size_t bytes = (size_t)h->C.R * 4;
+  if (cur_fit) TSA_CUDA(cudaMemcpyAsync(cur_fit, h->C.fit_cur, bytes, cudaMemcpyDeviceToHost, h->stream));
+  if (best_fit) TSA_CUDA(cudaMemcpyAsync(best_fit, h->C.fit_best, bytes, cudaMemcpyDeviceToHost, h->stream));
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  return SA_OK;
+}
+
+int sa_get_chain(sa_handle* h, int32_t chain, int8_t* cur, uint32_t* cur_fit, int8_t* best, uint32_t* best_fit) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  if (chain < 0 || chain >= h->C.R) return set_err(SA_EINVAL, "chain out of range");
+  const tsa::DevProblem& P = h->P;
+  std::vector<int8_t> w(P.EpadA), th(P.NpadA);
+  cudaStream_t st = h->stream;
+  if (cur) {
+    TSA_CUDA(cudaMemcpyAsync(w.data(), h->C.cur_w + (size_t)chain * P.EpadA, P.EpadA, cudaMemcpyDeviceToHost, st));
+    TSA_CUDA(cudaMemcpyAsync(th.data(), h->C.cur_th + (size_t)chain * P.NpadA, P.NpadA, cudaMemcpyDeviceToHost, st));
+    TSA_CUDA(cudaStreamSynchronize(st));
+    h->plan.to_caller(w.data(), th.data(), cur);
+  }
+  if (best) {
+    TSA_CUDA(cudaMemcpyAsync(w.data(), h->C.best_w + (size_t)chain * P.EpadA, P.EpadA, cudaMemcpyDeviceToHost, st));
+    TSA_CUDA(cudaMemcpyAsync(th.data(), h->C.best_th + (size_t)chain * P.NpadA, P.NpadA, cudaMemcpyDeviceToHost, st));
+    TSA_CUDA(cudaStreamSynchronize(st));
+    h->plan.to_caller(w.data(), th.data(), best);
+  }
+  if (cur_fit) TSA_CUDA(cudaMemcpyAsync(cur_fit, h->C.fit_cur + chain, 4, cudaMemcpyDeviceToHost, st));
+  if (best_fit) TSA_CUDA(cudaMemcpyAsync(best_fit, h->C.fit_best + chain, 4, cudaMemcpyDeviceToHost, st));
+  TSA_CUDA(cudaStreamSynchronize(st));
+  return SA_OK;
+}
+
+int sa_best(sa_handle* h, uint32_t* fitness, int32_t* chain, int8_t* params) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  DevPool tmp;
+  unsigned long long* d = (unsigned long long*)tmp.alloc(8, h->stream);
+  if (!d) return set_err(SA_ENOMEM, "device allocation failed");
+  TSA_CUDA(tsa::launch_argmin(h->C.fit_best, h->C.R, d, h->stream));
+  ++h->launches;
+  unsigned long long packed = 0;
+  TSA_CUDA(cudaMemcpyAsync(&packed, d, 8, cudaMemcpyDeviceToHost, h->stream));
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  const int32_t c = (int32_t)(packed & 0xFFFFFFFFull);
+  if (fitness) *fitness = (uint32_t)(packed >> 32);
+  if (chain) *chain = c;
+  if (params) return sa_get_chain(h, c, nullptr, nullptr, params, nullptr);
+  return SA_OK;
+}
+
+static int eval_sets(const tsa::Plan& pl, const tsa::DevProblem& P, const int8_t* params, int64_t n, uint32_t* fitness,
+                     uint8_t* dump_dev, int threads, cudaStream_t st, int64_t* launches) {
+  const int64_t kBatch = 65536;
+  DevPool tmp;
+  const int64_t cap = std::min(n, kBatch);
+  int8_t* dw = (int8_t*)tmp.alloc((size_t)cap * P.EpadA, st);
+  int8_t* dth = (int8_t*)tmp.alloc((size_t)cap * P.NpadA, st);
+  uint32_t* dfit = (uint32_t*)tmp.alloc((size_t)cap * 4, st);
+  if (!dw || !dth || !dfit) return set_err(SA_ENOMEM, "device allocation failed (eval)");
+  std::vector<int8_t> hw((size_t)cap * P.EpadA), hth((size_t)cap * P.NpadA);
+  for (int64_t a = 0; a < n; a += kBatch) {
+    const int64_t m = std::min(kBatch, n - a);
+    for (int64_t r = 0; r < m; ++r)
+      pl.to_internal(params + (a + r) * pl.P, hw.data() + r * P.EpadA, hth.data() + r * P.NpadA);
+    TSA_CUDA(cudaMemcpyAsync(dw, hw.data(), (size_t)m * P.EpadA, cudaMemcpyHostToDevice, st));
+    TSA_CUDA(cudaMemcpyAsync(dth, hth.data(), (size_t)m * P.NpadA, cudaMemcpyHostToDevice, st));
+    TSA_CUDA(tsa::launch_eval(P, dw, dth, m, dfit, dump_dev, threads, st));
+    if (launches) ++*launches;
+    if (fitness) TSA_CUDA(cudaMemcpyAsync(fitness + a, dfit, (size_t)m * 4, cudaMemcpyDeviceToHost, st));
+    TSA_CUDA(cudaStreamSynchronize(st));
+  }
+  return SA_OK;
+}
+
+int sa_eval(sa_handle* h, const int8_t* params, int64_t n, uint32_t* fitness) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  if (!params || !fitness || n < 0) return set_err(SA_EINVAL, "bad sa_eval arguments");
+  if (n == 0) return SA_OK;
+  if (!tsa::params_valid(h->plan, params, n)) return set_err(SA_EINVAL, "parameter value out of range");
+  return eval_sets(h->plan, h->P, params, n, fitness, nullptr, h->threads, h->stream, &h->launches);
+}
+
+int sa_simulate(const sa_network* net, const sa_observations* obs, const int8_t* params, uint8_t* states) {
+  if (!net || !obs || !params || !states) return set_err(SA_EINVAL, "null argument");
+  tsa::Plan pl;
+  std::string err;
+  int rc = tsa::build_plan(net, obs, false, &pl, &err);
+  if (rc != SA_OK) return set_err(rc, err);
+  if (!tsa::params_valid(pl, params, 1)) return set_err(SA_EINVAL, "parameter value out of range");
+  int dev = 0, sms = 148;
+  TSA_CUDA(cudaGetDevice(&dev));
+  TSA_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  DevPool pool;
+  tsa::DevProblem P;
+  cudaStream_t st = 0;
+  if ((rc = upload_problem(pl, pool, &P, st))) return rc;
+  if (tsa::smem_bytes(P) > 227 * 1024) return set_err(SA_EINVAL, "chain state does not fit shared memory");
+  const size_t out_bytes = (size_t)pl.K * pl.n_obs * pl.N;
+  uint8_t* d_out = (uint8_t*)pool.alloc(out_bytes, st);
+  if (!d_out) return set_err(SA_ENOMEM, "device allocation failed");
+  TSA_CUDA(cudaMemsetAsync(d_out, 0, out_bytes, st));
+  rc = eval_sets(pl, P, params, 1, nullptr, d_out, pick_threads(P, 1, sms), st, nullptr);
+  if (rc != SA_OK) return rc;
+  TSA_CUDA(cudaMemcpy(states, d_out, out_bytes, cudaMemcpyDeviceToHost));
+  return SA_OK;
+}
+
+int sa_set_trace(sa_handle* h, const int32_t* chains, int32_t n, int64_t max_steps) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  h->trace_pool.clear();
+  std::memset(&h->Tr, 0, sizeof(h->Tr));
+  h->n_traced = 0;
+  h->trace_steps = 0;
+  if (n == 0) return SA_OK;
+  if (n < 0 || !chains || max_steps <= 0) return set_err(SA_EINVAL, "bad sa_set_trace arguments");
+  std::vector<int32_t> row(h->C.R, -1);
+  for (int32_t i = 0; i < n; ++i) {
+    if (chains[i] < 0 || chains[i] >= h->C.R) return set_err(SA_EINVAL, "traced chain out of range");
+    if (row[chains[i]] != -1) return set_err(SA_EINVAL, "traced chain listed twice");
+    row[chains[i]] = i;
+  }
+  const int32_t* d_row = nullptr;
+  int rc = h->trace_pool.upload(row, &d_row, h->stream);
+  if (rc) return rc;
+  const size_t bytes = (size_t)n * (size_t)max_steps * 8;
+  uint64_t* rec = (uint64_t*)h->trace_pool.alloc(bytes, h->stream);
+  if (!rec) { h->trace_pool.clear(); return set_err(SA_ENOMEM, "device allocation failed (trace)"); }
+  TSA_CUDA(cudaMemsetAsync(rec, 0, bytes, h->stream));
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  h->Tr.row_of_chain = d_row;
+  h->Tr.records = rec;
+  h->Tr.max_steps = max_steps;
+  h->Tr.g_start = h->g;
+  h->n_traced = n;
+  h->trace_steps = max_steps;
+  return SA_OK;
+}
+
+int sa_get_trace(sa_handle* h, uint64_t* records) {
+  if (!h || !records) return set_err(SA_EINVAL, "null argument");
+  if (h->n_traced == 0) return set_err(SA_EINVAL, "tracing is off");
+  const size_t bytes = (size_t)h->n_traced * (size_t)h->trace_steps * 8;
+  TSA_CUDA(cudaMemcpyAsync(records, h->Tr.records, bytes, cudaMemcpyDeviceToHost, h->stream));
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  return SA_OK;
+}
+
+int sa_get_info(sa_handle* h, int64_t info[8]) {
+  if (!h || !info) return set_err(SA_EINVAL, "null argument");
+  info[0] = 1;                                   // kernel variant: 1 = generic CTA-per-chain
+  info[1] = h->threads;
+  info[2] = 1;
+  info[3] = (int64_t)tsa::smem_bytes(h->P);
+  info[4] = h->C.R;
+  info[5] = h->P.Epad;
+  info[6] = h->sm_count;
+  info[7] = h->launches;
+  return SA_OK;
+}
+
+}  // extern "C"

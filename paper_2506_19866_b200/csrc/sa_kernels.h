@@ -1,0 +1,20 @@
+// Launch wrappers of the CUDA kernels (sa_kernels.cu).  Internal to libternary_sa.so.
+#pragma once
+#include <cuda_runtime.h>
+
+#include "sa_common.h"
+
+namespace tsa {
+
+size_t smem_bytes(const DevProblem& P);
+
+// one CTA of `threads` threads per chain / parameter set
+cudaError_t launch_init(const DevProblem& P, const DevChains& C, const DevSched& S, int threads, cudaStream_t st);
+cudaError_t launch_run(const DevProblem& P, const DevChains& C, const DevSched& S, const DevTrace& Tr,
+                       uint64_t g0, int64_t steps, int threads, cudaStream_t st);
+cudaError_t launch_eval(const DevProblem& P, const int8_t* w, const int8_t* th, int64_t n, uint32_t* fit,
+                        uint8_t* dump, int threads, cudaStream_t st);
+// out[0] = (fitness << 32) | chain of the best chain (smallest fitness, then smallest index)
+cudaError_t launch_argmin(const uint32_t* fit, int R, unsigned long long* out, cudaStream_t st);
+
+}  // namespace tsa

@@ -1,0 +1,102 @@
+"""Host-side checks of the C-ABI library that need no GPU: it loads, exports every symbol the
+header declares, validates its inputs, and its host helper matches the pinned table values."""
+import copy
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+from helpers import golden_rows
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2506_19866_b200 import build
+    build.build()
+    from paper_2506_19866_b200 import binding
+    return binding
+
+
+def _declared_functions():
+    text = open(os.path.join(ROOT, "include", "ternary_sa.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(sa_[a-z0-9_]+)\s*\(", text)) - {"sa_alloc_fn", "sa_free_fn"})
+
+
+def test_library_exports_every_declared_symbol(B):
+    names = _declared_functions()
+    assert len(names) >= 16
+    lib = ctypes.CDLL(B.LIB_PATH)
+    for n in names:
+        assert hasattr(lib, n), f"{n} is declared in include/ternary_sa.h but not exported"
+    assert sorted(B.EXPORTS) == names
+
+
+def test_geometric_table_helper_matches_pins(B):
+    for T, d, want in golden_rows("accept_table.txt"):
+        tab = B.sa_geometric_table(float(T), float(T), 1, 64)
+        assert int(tab[0, int(d) - 1]) == int(want)
+    from paper_2506_19866_b200 import problems as PB
+    assert np.array_equal(B.sa_geometric_table(PB.T0, PB.T_END, PB.N_LEVELS, PB.DMAX),
+                          PB.geometric_table(PB.T0, PB.T_END, PB.N_LEVELS, PB.DMAX))
+    with pytest.raises(B.SaError):
+        B.sa_geometric_table(-1.0, 1.0, 4, 4)
+
+
+def _bad(B, prob, sched, match):
+    with pytest.raises(B.SaError) as ei:
+        B.sa_create(prob, sched)
+    assert ei.value.code == B.SA_EINVAL and match in str(ei.value), str(ei.value)
+
+
+def test_sa_create_validation(B, problems_cache):
+    from paper_2506_19866_b200 import problems as PB
+    good = problems_cache("tiny")
+    sched = PB.default_schedule("tiny")
+
+    p = copy.copy(good); p.edge_src = good.edge_src.copy(); p.edge_src[0] = p.edge_dst[0]
+    _bad(B, p, sched, "self-loop")
+    p = copy.copy(good); p.edge_src = good.edge_src.copy(); p.edge_dst = good.edge_dst.copy()
+    p.edge_src[1], p.edge_dst[1] = p.edge_src[0], p.edge_dst[0]
+    _bad(B, p, sched, "duplicate")
+    p = copy.copy(good); p.edge_dst = good.edge_dst.copy(); p.edge_dst[0] = good.n_nodes
+    _bad(B, p, sched, "out of range")
+    p = copy.copy(good); p.th_lo = good.th_lo.copy(); p.th_lo[2] = 0
+    _bad(B, p, sched, "th_lo")
+    p = copy.copy(good); p.init_state = good.init_state.copy(); p.init_state[0, 0] = 3
+    _bad(B, p, sched, "init_state")
+    p = copy.copy(good); p.obs = good.obs.copy(); p.obs[0, 0, 0] = 7
+    _bad(B, p, sched, "obs must")
+    p = copy.copy(good); p.obs_times = np.array([3, 3, 9, 12], dtype=np.int32)
+    _bad(B, p, sched, "obs_times")
+    p = copy.copy(good); p.obs_times = np.array([3, 6, 9, 13], dtype=np.int32)
+    _bad(B, p, sched, "obs_times")
+    s = copy.copy(sched); s.n_chains = 0
+    _bad(B, good, s, "schedule")
+    # accumulator range: a node with in-degree 63 is refused (reading 24)
+    N = 65
+    star = copy.copy(good)
+    star.n_nodes, star.n_edges = N, 63
+    star.edge_src = np.arange(1, 64, dtype=np.int32); star.edge_dst = np.zeros(63, dtype=np.int32)
+    star.init_state = np.zeros((good.n_cond, N), dtype=np.uint8); star.clamp = np.zeros((good.n_cond, N), dtype=np.uint8)
+    star.obs = np.full((good.n_cond, good.n_obs, N), 255, dtype=np.uint8)
+    _bad(B, star, sched, "accumulator")
+
+
+def test_no_cpu_fallback(B, problems_cache):
+    """Without a CUDA device the product path must fail loudly, not compute on the host."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2506_19866_b200 import problems as PB
+    with pytest.raises(B.SaError) as ei:
+        B.sa_create(problems_cache("tiny"), PB.default_schedule("tiny"))
+    assert ei.value.code in (B.SA_ECUDA, B.SA_ENOMEM)
+    with pytest.raises(B.SaError):
+        B.sa_simulate(problems_cache("tiny"), problems_cache("tiny").truth)
+    assert B.sa_run.__doc__ is None or True
+    B.sa_destroy(None)                      # NULL is a no-op

@@ -1,0 +1,329 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle — bit-exact, element by
+element, on the same seeded inputs.  Everything here needs a GPU (-m gpu)."""
+import copy
+import os
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_2506_19866_b200 import problems as PB
+from helpers import all_settings, brute_force_problem, example_problem
+
+pytestmark = pytest.mark.gpu
+NCPU = max(1, min(32, os.cpu_count() or 1))
+
+
+@pytest.fixture(scope="module")
+def B():
+    import torch
+    assert torch.cuda.is_available(), "the gpu tests need a CUDA device"
+    from paper_2506_19866_b200 import build
+    build.build()
+    from paper_2506_19866_b200 import binding
+    binding.use_torch_plumbing()
+    return binding
+
+
+class Handle:
+    def __init__(self, B, prob, sched):
+        self.B, self.prob, self.sched = B, prob, sched
+        self.h = B.sa_create(prob, sched)
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *a):
+        self.B.sa_destroy(self.h)
+
+
+def oracle_chains(orc, sched, chains, n_steps):
+    with ThreadPoolExecutor(NCPU) as ex:
+        return list(ex.map(lambda c: orc.run_chain(sched, c + sched.chain_id_base, n_steps), chains))
+
+
+def check_chains(B, hd, orc, chains, n_steps, trace=None):
+    """GPU state of `chains` after n_steps from a fresh handle == oracle (trace, vectors, fitness)."""
+    refs = oracle_chains(orc, hd.sched, chains, n_steps)
+    for row, (c, ref) in enumerate(zip(chains, refs)):
+        cur, fc, best, fb = B.sa_get_chain(hd.h, c, hd.prob.n_params)
+        if trace is not None:
+            bad = np.nonzero(trace[row][:n_steps] != ref["trace"])[0]
+            assert bad.size == 0, f"chain {c}: first trace mismatch at step {bad[0]}: " \
+                                  f"gpu {int(trace[row][bad[0]]):#x} oracle {int(ref['trace'][bad[0]]):#x}"
+        assert (fc, fb) == (ref["fit_cur"], ref["fit_best"]), f"chain {c} fitness"
+        assert np.array_equal(cur, ref["cur"]), f"chain {c} current vector"
+        assert np.array_equal(best, ref["best"]), f"chain {c} best vector"
+
+
+def check_all_fitness(B, hd, orc):
+    """For every chain: reported d_cur / d_best equal the ORACLE fitness of the returned vectors."""
+    R, P = hd.sched.n_chains, hd.prob.n_params
+    fcur, fbest = B.sa_get_fitness(hd.h, R)
+    assert (fbest <= fcur).all()
+    cur = np.zeros((R, P), dtype=np.int8)
+    best = np.zeros((R, P), dtype=np.int8)
+    for c in range(R):
+        cur[c], fc, best[c], fb = B.sa_get_chain(hd.h, c, P)
+        assert fc == fcur[c] and fb == fbest[c]
+    assert np.array_equal(orc.fitness_batch(cur, threads=NCPU), fcur)
+    assert np.array_equal(orc.fitness_batch(best, threads=NCPU), fbest)
+    fit, chain, params = B.sa_best(hd.h, P)
+    assert fit == fbest.min() and chain == int(np.argmin(fbest)) and np.array_equal(params, best[chain])
+
+
+# --------------------------------------------------------------------------------- fitness
+@pytest.mark.parametrize("name,count", [("tiny", 256), ("hpg", 256), ("mtb", 128), ("large", 12)])
+def test_eval_and_simulate_match_oracle(B, problems_cache, name, count):
+    prob = problems_cache(name)
+    orc = O.Oracle(prob)
+    assert np.array_equal(B.sa_simulate(prob, prob.truth), orc.states_at_obs(prob.truth))
+    X = np.concatenate([PB.random_params(prob, count, seed=21), prob.truth[None, :]])
+    with Handle(B, prob, PB.default_schedule(name, n_chains=4)) as hd:
+        got = B.sa_eval(hd.h, X)
+    want = orc.fitness_batch(X, threads=NCPU)
+    assert np.array_equal(got, want)
+    assert got[-1] == prob.n_flipped
+
+
+def test_eval_hand_worked_examples(B):
+    prob = example_problem(with_condition_b=True)
+    sched = PB.make_schedule(2, 100)
+    X = np.stack([prob.truth] * 4)
+    X[1, 0] = 0; X[2, 7] = 5; X[3, 4] = 1
+    with Handle(B, prob, sched) as hd:
+        assert B.sa_eval(hd.h, X).tolist() == [1, 2, 5, 2]          # tests/golden/example_b_fitness.txt
+    probA = example_problem()
+    assert np.array_equal(B.sa_simulate(probA, probA.truth), O.Oracle(probA).states_at_obs(probA.truth))
+
+
+def test_eval_brute_force_every_setting(B):
+    prob = brute_force_problem(O.simulate_fn)
+    X = all_settings(6, 4, 6)
+    want = O.Oracle(prob).fitness_batch(X, threads=NCPU)
+    with Handle(B, prob, PB.make_schedule(2, 100)) as hd:
+        got = B.sa_eval(hd.h, X)
+    assert np.array_equal(got, want)                                # all 944 784 elements
+
+
+# --------------------------------------------------------------------------------- SA runs
+def test_tiny_full_parity(B, problems_cache):
+    prob = problems_cache("tiny")
+    sched = PB.default_schedule("tiny")
+    orc = O.Oracle(prob)
+    chains = list(range(8))
+    with Handle(B, prob, sched) as hd:
+        f0, _ = B.sa_get_fitness(hd.h, 8)
+        assert f0.tolist() == [orc.init_chain(sched.seed, c)[1] for c in chains]
+        B.sa_set_trace(hd.h, chains, 2000)
+        B.sa_run(hd.h, 2000)
+        check_chains(B, hd, orc, chains, 2000, B.sa_get_trace(hd.h, 8, 2000))
+        check_all_fitness(B, hd, orc)
+
+
+def test_hpg_full_size_parity(B, problems_cache):
+    prob = problems_cache("hpg")
+    sched = PB.default_schedule("hpg")                                # R = 1024, 20 000 steps
+    orc = O.Oracle(prob)
+    chains = PB.spread_chains(1024, 48)
+    with Handle(B, prob, sched) as hd:
+        B.sa_set_trace(hd.h, chains, 20000)
+        B.sa_run(hd.h, 20000)
+        check_chains(B, hd, orc, chains, 20000, B.sa_get_trace(hd.h, len(chains), 20000))
+        check_all_fitness(B, hd, orc)
+    with Handle(B, prob, sched) as hd:                                # every chain, first 200 steps
+        B.sa_run(hd.h, 200)
+        check_chains(B, hd, orc, list(range(1024)), 200)
+
+
+def test_mtb_full_size_parity(B, problems_cache):
+    prob = problems_cache("mtb")
+    sched = PB.default_schedule("mtb")                                # R = 4096, 20 000 steps
+    orc = O.Oracle(prob)
+    long_chains = [0, 4095]
+    short_chains = PB.spread_chains(4096, 14)
+    with Handle(B, prob, sched) as hd:
+        f0, _ = B.sa_get_fitness(hd.h, 4096)
+        B.sa_set_trace(hd.h, sorted(set(long_chains + short_chains)), 20000)
+        traced = sorted(set(long_chains + short_chains))
+        B.sa_run(hd.h, 20000)
+        trace = B.sa_get_trace(hd.h, len(traced), 20000)
+        check_chains(B, hd, orc, long_chains, 20000, trace[[traced.index(c) for c in long_chains]])
+        refs = oracle_chains(orc, sched, short_chains, 2500)          # trace prefix of more chains
+        for c, ref in zip(short_chains, refs):
+            assert np.array_equal(trace[traced.index(c)][:2500], ref["trace"]), f"chain {c}"
+            assert f0[c] == ref["init_fit"]
+        check_all_fitness(B, hd, orc)
+    with Handle(B, prob, sched) as hd:                                # every chain, first 20 steps
+        B.sa_run(hd.h, 20)
+        check_chains(B, hd, orc, list(range(4096)), 20)
+
+
+def test_scaling_chain_counts(B, problems_cache):
+    prob = problems_cache("mtb")
+    orc = O.Oracle(prob)
+    common = [0, 1, 500, 1023]
+    traces = {}
+    for R in PB.SCALING_CHAINS:
+        sched = PB.default_schedule("mtb", n_chains=R, total_steps=PB.SCALING_STEPS)
+        chains = sorted(set(common + PB.spread_chains(R, 8)))
+        with Handle(B, prob, sched) as hd:
+            B.sa_set_trace(hd.h, chains, 2000)
+            B.sa_run(hd.h, 2000)
+            tr = B.sa_get_trace(hd.h, len(chains), 2000)
+            check_chains(B, hd, orc, chains, 2000, tr)
+            traces[R] = {c: tr[chains.index(c)] for c in common}
+            if R == 1024:
+                check_all_fitness(B, hd, orc)
+    for c in common:                                                  # invariant (vii): independent of R
+        assert np.array_equal(traces[1024][c], traces[8192][c]) and np.array_equal(traces[1024][c], traces[65536][c])
+    sched = PB.default_schedule("mtb", n_chains=65536, total_steps=PB.SCALING_STEPS)
+    with Handle(B, prob, sched) as hd:                                # all chains x 2 steps (sampled 1 in 16)
+        B.sa_run(hd.h, 2)
+        check_chains(B, hd, orc, list(range(0, 65536, 16)), 2)
+
+
+def test_large_parity(B, problems_cache):
+    prob = problems_cache("large")
+    sched = PB.default_schedule("large")                              # R = 2048, 1000 steps
+    orc = O.Oracle(prob)
+    chains = PB.spread_chains(2048, 8)
+    with Handle(B, prob, sched) as hd:
+        f0, _ = B.sa_get_fitness(hd.h, 2048)
+        with ThreadPoolExecutor(NCPU) as ex:
+            want0 = list(ex.map(lambda c: orc.init_chain(sched.seed, c)[1], range(2048)))
+        assert f0.tolist() == want0                                   # all chains: initial fitness
+        B.sa_set_trace(hd.h, chains, 1000)
+        B.sa_run(hd.h, 1000)
+        check_chains(B, hd, orc, chains, 1000, B.sa_get_trace(hd.h, len(chains), 1000))
+    with Handle(B, prob, sched) as hd:                                # all chains: one step
+        B.sa_run(hd.h, 1)
+        check_chains(B, hd, orc, list(range(0, 2048, 4)), 1)
+
+
+# --------------------------------------------------------------------------------- invariants
+def test_split_runs_chain_base_and_team_width(B, problems_cache):
+    prob = problems_cache("mtb")
+    sched = PB.default_schedule("mtb", n_chains=16, total_steps=600)
+    with Handle(B, prob, sched) as a:
+        B.sa_set_trace(a.h, list(range(16)), 600)
+        B.sa_run(a.h, 600)
+        ta = B.sa_get_trace(a.h, 16, 600)
+        state_a = [B.sa_get_chain(a.h, c, prob.n_params) for c in range(16)]
+    with Handle(B, prob, sched) as b:                                 # run(a); run(b) == run(a+b)
+        B.sa_set_trace(b.h, list(range(16)), 600)
+        for part in (1, 99, 250, 250):
+            B.sa_run(b.h, part)
+        assert np.array_equal(B.sa_get_trace(b.h, 16, 600), ta)
+    part_sched = copy.copy(sched); part_sched.n_chains = 4; part_sched.chain_id_base = 8
+    with Handle(B, prob, part_sched) as c:                            # chain-range partition (reading 25)
+        B.sa_set_trace(c.h, [0, 1, 2, 3], 600)
+        B.sa_run(c.h, 600)
+        assert np.array_equal(B.sa_get_trace(c.h, 4, 600), ta[8:12])
+    for warps in ("1", "2", "4"):                                     # launch geometry never changes results
+        os.environ["TSA_TEAM_WARPS"] = warps
+        try:
+            with Handle(B, prob, sched) as d:
+                assert B.sa_get_info(d.h)["threads_per_cta"] == 32 * int(warps)
+                B.sa_run(d.h, 600)
+                for ch in range(16):
+                    got = B.sa_get_chain(d.h, ch, prob.n_params)
+                    assert np.array_equal(got[0], state_a[ch][0]) and got[1] == state_a[ch][1]
+                    assert np.array_equal(got[2], state_a[ch][2]) and got[3] == state_a[ch][3]
+        finally:
+            del os.environ["TSA_TEAM_WARPS"]
+
+
+def test_extreme_tables(B, problems_cache):
+    prob = problems_cache("hpg")
+    orc = O.Oracle(prob)
+    greedy = PB.make_schedule(8, 400)
+    greedy.accept = np.zeros_like(greedy.accept)
+    hot = PB.make_schedule(8, 400, dmax=prob.n_scored)
+    hot.accept = np.full((hot.n_levels, prob.n_scored), 0xFFFFFFFF, dtype=np.uint32)
+    for sched in (greedy, hot):
+        with Handle(B, prob, sched) as hd:
+            B.sa_set_trace(hd.h, list(range(8)), 400)
+            B.sa_run(hd.h, 400)
+            check_chains(B, hd, orc, list(range(8)), 400, B.sa_get_trace(hd.h, 8, 400))
+    # past the end of the schedule the level saturates at L-1 (reading 20)
+    short = PB.make_schedule(4, 200, n_levels=10)
+    with Handle(B, prob, short) as hd:
+        B.sa_set_trace(hd.h, [0, 1, 2, 3], 500)
+        B.sa_run(hd.h, 500)
+        check_chains(B, hd, orc, [0, 1, 2, 3], 500, B.sa_get_trace(hd.h, 4, 500))
+
+
+# --------------------------------------------------------------------------------- edge cases
+EDGE_SPECS = [
+    # name            N   E   degree           K  clamp T  obs_times
+    ("k1",            9,  20, "uniform-pairs", 1, 1,    5, (1, 5)),
+    ("k5_pad_lanes",  12, 40, "poisson",       5, 2,    7, (2, 4, 7)),
+    ("k9",            20, 70, "poisson",       9, 1,    6, (3, 6)),
+    ("k17_chunks",    10, 30, "uniform-pairs", 17, 1,   6, (2, 6)),
+    ("k37_chunks",    8,  24, "uniform-pairs", 37, 2,   4, (1, 2, 3, 4)),
+    ("n33_two_pass",  33, 120, "poisson",      4, 3,    8, (4, 8)),
+    ("n70_ragged",    70, 400, "powerlaw",     6, 2,    9, (3, 6, 9)),
+    ("t1",            16, 50, "poisson",       3, 1,    1, (1,)),
+    ("all_clamped",   6,  12, "uniform-pairs", 2, 6,    4, (2, 4)),
+    ("sparse",        40, 41, "uniform-pairs", 8, 1,    10, (5, 10)),
+]
+
+
+@pytest.mark.parametrize("spec", EDGE_SPECS, ids=[s[0] for s in EDGE_SPECS])
+def test_edge_shapes(B, spec):
+    name, N, E, degree, K, nclamp, T, times = spec
+    cs = PB.ConfigSpec(name, 4242 + N + K, N, E, degree, K, nclamp, T, times, 12, 300,
+                       max_in_degree=min(N - 1, 40))
+    prob = PB.make_problem(name, O.simulate_fn, spec=cs, noise=0.10)
+    orc = O.Oracle(prob)
+    sched = PB.make_schedule(12, 300)
+    X = PB.random_params(prob, 64, seed=N)
+    with Handle(B, prob, sched) as hd:
+        assert np.array_equal(B.sa_eval(hd.h, X), orc.fitness_batch(X))
+        assert np.array_equal(B.sa_simulate(prob, prob.truth), orc.states_at_obs(prob.truth))
+        B.sa_set_trace(hd.h, list(range(12)), 300)
+        B.sa_run(hd.h, 300)
+        check_chains(B, hd, orc, list(range(12)), 300, B.sa_get_trace(hd.h, 12, 300))
+        check_all_fitness(B, hd, orc)
+
+
+def test_nothing_observed_and_max_in_degree(B):
+    # nothing observed: fitness is 0 for everything, every move has d = 0 and is accepted
+    cs = PB.ConfigSpec("blind", 99, 10, 30, "uniform-pairs", 3, 1, 5, (2, 5), 4, 100)
+    prob = PB.make_problem("blind", O.simulate_fn, spec=cs)
+    prob.obs = np.full_like(prob.obs, 255)
+    sched = PB.make_schedule(4, 100)
+    orc = O.Oracle(prob)
+    with Handle(B, prob, sched) as hd:
+        B.sa_set_trace(hd.h, [0, 1, 2, 3], 100)
+        B.sa_run(hd.h, 100)
+        tr = B.sa_get_trace(hd.h, 4, 100)
+        assert O.unpack_trace(tr)["accepted"].all() and (O.unpack_trace(tr)["delta_cand"] == 0).all()
+        check_chains(B, hd, orc, [0, 1, 2, 3], 100, tr)
+    # a hub with in-degree 62 (the accumulator limit) fed by nodes stuck at 2: sums reach +-124
+    N = 64
+    star = copy.copy(prob)
+    star.n_nodes, star.n_edges = N, 62 + 1
+    star.edge_src = np.array(list(range(1, 63)) + [0], dtype=np.int32)
+    star.edge_dst = np.array([0] * 62 + [63], dtype=np.int32)
+    star.init_state = np.full((3, N), 2, dtype=np.uint8)
+    star.clamp = np.ones((3, N), dtype=np.uint8); star.clamp[:, 0] = 0; star.clamp[:, 63] = 0
+    star.obs = np.full((3, 2, N), 255, dtype=np.uint8); star.obs[:, :, 0] = 1; star.obs[:, :, 63] = 2
+    orc = O.Oracle(star)
+    X = PB.random_params(star, 40, seed=5)
+    X[0, :63] = 1; X[1, :63] = -1; X[2, :62] = 1; X[2, 62] = -1
+    with Handle(B, star, sched) as hd:
+        assert np.array_equal(B.sa_eval(hd.h, X), orc.fitness_batch(X))
+        B.sa_run(hd.h, 100)
+        check_chains(B, hd, orc, [0, 1, 2, 3], 100)
+
+
+def test_int32_peak_microbenchmark_runs(B):
+    pk = B.sa_int32_peak()
+    assert pk["sm_count"] > 0 and pk["sm_hz"] > 2e8
+    for k in ("iadd3", "lop3", "imad", "mixed"):
+        # never above one instruction per scheduler per clock, never absurdly low
+        ceiling = pk["sm_count"] * 4 * pk["sm_hz"]
+        assert 0.05 * ceiling < pk[k] < 1.05 * ceiling, (k, pk)
