@@ -119,9 +119,17 @@ int sa_geometric_table(double t0, double t_end, int32_t n_levels, int32_t dmax, 
 
 /* Which kernel family a handle uses and how it was launched (for bench.py / DESIGN.md):
  * info[0] = kernel variant id, [1] = threads per CTA, [2] = chains per CTA, [3] = dynamic shared
- * memory bytes per CTA, [4] = CTAs in the sa_run grid, [5] = padded edge slots, [6] = SM count,
- * [7] = kernels launched so far by this handle. */
-int sa_get_info(sa_handle *h, int64_t info[8]);
+ * memory bytes per CTA, [4] = CTAs in the sa_run grid, [5] = edge slots per chain (padded),
+ * [6] = SM count, [7] = kernels launched so far by this handle, [8] = passes per time step,
+ * [9] = edge iterations per time step (sum over passes), [10] = rows, [11] = split nodes,
+ * [12] = state words per node, [13] = state entries; the rest is 0. */
+int sa_get_info(sa_handle *h, int64_t info[16]);
+
+/* Host only (no GPU needed): build the execution plan of a problem and report its shape in the
+ * same slots as sa_get_info ([0], [5], [8]-[13]), plus [14] = max in-degree, [15] = number of
+ * mismatches contributed by clamped observed entries (constant over all parameter sets).
+ * obs->obs may be NULL.  Fails like sa_create on invalid input. */
+int sa_plan_info(const sa_network *net, const sa_observations *obs, int64_t info[16]);
 
 /* ---- plumbing ---- */
 

@@ -71,22 +71,32 @@ int upload_problem(const tsa::Plan& pl, DevPool& pool, tsa::DevProblem* P, cudaS
   tsa::DevProblem& d = *P;
   std::memset(&d, 0, sizeof(d));
   d.N = pl.N; d.E = pl.E; d.P = pl.P; d.K = pl.K; d.T = pl.T; d.n_obs = pl.n_obs; d.n_pairs = pl.n_pairs;
-  d.CG = pl.CG; d.n_chunks = pl.n_chunks; d.n_pass = pl.n_pass; d.Epad = pl.Epad; d.EpadA = pl.EpadA;
-  d.NpadA = pl.NpadA; d.state_words = pl.state_words;
+  d.CG = pl.CG; d.n_chunks = pl.n_chunks; d.n_pass = pl.n_pass; d.n_entries = pl.n_entries;
+  d.Epad = pl.Epad; d.EpadA = pl.EpadA; d.NpadA = pl.NpadA; d.state_words = pl.state_words;
+  d.fit_const = pl.fit_const;
+  d.n_fix = (int)pl.fix.size();
   std::memcpy(d.tha, pl.tha, sizeof(d.tha));
   std::memcpy(d.thb, pl.thb, sizeof(d.thb));
+  std::vector<int4> info((size_t)pl.n_chunks * pl.n_pass);
+  for (int ch = 0; ch < pl.n_chunks; ++ch)
+    for (int ps = 0; ps < pl.n_pass; ++ps) {
+      const size_t x = (size_t)ch * pl.n_pass + ps;
+      info[x] = make_int4(pl.pass_base[ps], pl.pass_iters[ps] | (pl.pass_rounds[ps] << 16), pl.fix_ptr[x],
+                          pl.fix_ptr[x + 1] - pl.fix_ptr[x]);
+    }
   int rc;
-  if ((rc = pool.upload(pl.pass_base, &d.pass_base, st))) return rc;
-  if ((rc = pool.upload(pl.pass_deg, &d.pass_deg, st))) return rc;
+  if ((rc = pool.upload(info, &d.pass_info, st))) return rc;
+  if ((rc = pool.upload(pl.row_meta, &d.row_meta, st))) return rc;
   if ((rc = pool.upload(pl.slot_off, &d.slot_off, st))) return rc;
   if ((rc = pool.upload(pl.slot_of_param, &d.slot_of_param, st))) return rc;
-  if ((rc = pool.upload(pl.row_of_node, &d.row_of_node, st))) return rc;
-  if ((rc = pool.upload(pl.node_of_row, &d.node_of_row, st))) return rc;
+  if ((rc = pool.upload(pl.entry_of_node, &d.entry_of_node, st))) return rc;
   if ((rc = pool.upload(pl.initw, &d.initw, st))) return rc;
-  if ((rc = pool.upload(pl.clampm, &d.clampm, st))) return rc;
   if ((rc = pool.upload(pl.obsw, &d.obsw, st))) return rc;
   if ((rc = pool.upload(pl.obsm, &d.obsm, st))) return rc;
+  if ((rc = pool.upload(pl.fix, &d.fix, st))) return rc;
   if ((rc = pool.upload(pl.obs_idx_of_t, &d.obs_idx_of_t, st))) return rc;
+  // the host vector `info` must outlive the async copy
+  if (cudaStreamSynchronize(st) != cudaSuccess) return set_err(SA_ECUDA, "upload failed");
   return SA_OK;
 }
 
@@ -105,6 +115,38 @@ int pick_threads(const tsa::DevProblem& P, int64_t n_ctas, int sm_count) {
   return 32 * warps;
 }
 
+// WarpTeam launch shape: chains per CTA that minimises the busiest SM's chain count (all chains run
+// the same number of steps, so the makespan is set by the fullest SM), larger CTAs on ties.
+// Returns 0 when the warp-per-chain kernel does not apply.
+int pick_warp_cpb(const tsa::DevProblem& P, int64_t R, int sm_count) {
+  if (const char* env = std::getenv("TSA_KERNEL")) {
+    if (std::string(env) == "cta") return 0;
+    if (std::string(env) == "warp" && P.n_pass <= 32) {
+      int cpb = 8;
+      if (const char* c = std::getenv("TSA_CPB")) cpb = std::max(1, std::min(8, std::atoi(c)));
+      return tsa::warp_kernel_smem(P, cpb) <= 227 * 1024 ? cpb : 0;
+    }
+  }
+  if (P.n_pass > 8) return 0;                                   // one warp per chain would be too slow
+  if (P.n_pass > 1 && R < 16LL * sm_count) return 0;            // few chains: spread each over a CTA
+  int best = 0;
+  int64_t best_load = 0;
+  for (int cpb = 8; cpb >= 1; --cpb) {
+    const size_t sb = tsa::warp_kernel_smem(P, cpb);
+    if (sb > 227 * 1024) continue;
+    const int64_t ctas = (R + cpb - 1) / cpb;
+    const int64_t fit = std::min<int64_t>(32, (int64_t)((228 * 1024) / (sb + 1024)));
+    if (fit < 1) continue;
+    const int64_t per_sm = (ctas + sm_count - 1) / sm_count;
+    const int64_t load = (per_sm <= fit) ? per_sm * cpb                      // single wave: static imbalance
+                                         : (R + sm_count - 1) / sm_count + cpb;   // several waves: dynamic, ~even
+    const int64_t resident = std::min(per_sm, fit) * cpb;
+    if (resident < std::min<int64_t>(16, (R + sm_count - 1) / sm_count)) continue;   // keep >= 16 warps per SM if possible
+    if (best == 0 || load < best_load) { best = cpb; best_load = load; }
+  }
+  return best;
+}
+
 }  // namespace
 
 struct sa_handle {
@@ -118,6 +160,7 @@ struct sa_handle {
   cudaStream_t stream = 0;
   uint64_t g = 0;       // global step counter
   int threads = 32;
+  int warp_cpb = 0;     // > 0: sa_run uses the warp-per-chain kernel with this many chains per CTA
   int sm_count = 148;
   int64_t launches = 0;
   int32_t n_traced = 0;
@@ -156,7 +199,7 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
   std::unique_ptr<sa_handle> h(new (std::nothrow) sa_handle());
   if (!h) return set_err(SA_ENOMEM, "host allocation failed");
   std::string err;
-  int rc = tsa::build_plan(net, obs, true, &h->plan, &err);
+  int rc = tsa::build_plan(net, obs, true, tsa::PlanOptions::from_env(), &h->plan, &err);
   if (rc != SA_OK) return set_err(rc, err);
 
   int dev = 0;
@@ -190,6 +233,7 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
   const size_t sb = tsa::smem_bytes(h->P);
   if (sb > 227 * 1024) return set_err(SA_EINVAL, "chain state does not fit shared memory (N, E too large for this kernel family)");
   h->threads = pick_threads(h->P, R, h->sm_count);
+  h->warp_cpb = pick_warp_cpb(h->P, R, h->sm_count);
   TSA_CUDA(tsa::launch_init(h->P, h->C, h->S, h->threads, st));
   ++h->launches;
   TSA_CUDA(cudaStreamSynchronize(st));   // host vectors used by the async uploads die with this frame
@@ -214,7 +258,10 @@ int sa_run(sa_handle* h, int64_t steps) {
   if (!h) return set_err(SA_EINVAL, "null handle");
   if (steps < 0) return set_err(SA_EINVAL, "steps < 0");
   if (steps == 0) return SA_OK;
-  TSA_CUDA(tsa::launch_run(h->P, h->C, h->S, h->Tr, h->g, steps, h->threads, h->stream));
+  if (h->warp_cpb > 0)
+    TSA_CUDA(tsa::launch_run_warp(h->P, h->C, h->S, h->Tr, h->g, steps, h->warp_cpb, h->stream));
+  else
+    TSA_CUDA(tsa::launch_run(h->P, h->C, h->S, h->Tr, h->g, steps, h->threads, h->stream));
   ++h->launches;
   h->g += (uint64_t)steps;
   return SA_OK;
@@ -306,7 +353,7 @@ int sa_simulate(const sa_network* net, const sa_observations* obs, const int8_t*
   if (!net || !obs || !params || !states) return set_err(SA_EINVAL, "null argument");
   tsa::Plan pl;
   std::string err;
-  int rc = tsa::build_plan(net, obs, false, &pl, &err);
+  int rc = tsa::build_plan(net, obs, false, tsa::PlanOptions::from_env(), &pl, &err);
   if (rc != SA_OK) return set_err(rc, err);
   if (!tsa::params_valid(pl, params, 1)) return set_err(SA_EINVAL, "parameter value out of range");
   int dev = 0, sms = 148;
@@ -368,16 +415,44 @@ int sa_get_trace(sa_handle* h, uint64_t* records) {
   return SA_OK;
 }
 
-int sa_get_info(sa_handle* h, int64_t info[8]) {
+int sa_plan_info(const sa_network* net, const sa_observations* obs, int64_t info[16]) {
+  if (!net || !obs || !info) return set_err(SA_EINVAL, "null argument");
+  tsa::Plan pl;
+  std::string err;
+  const int rc = tsa::build_plan(net, obs, obs->obs != nullptr, tsa::PlanOptions::from_env(), &pl, &err);
+  if (rc != SA_OK) return set_err(rc, err);
+  for (int i = 0; i < 16; ++i) info[i] = 0;
+  info[0] = 2;
+  info[5] = pl.Epad;
+  info[8] = pl.n_pass;
+  info[9] = pl.total_iters;
+  info[10] = pl.n_rows;
+  info[11] = pl.n_split_nodes;
+  info[12] = pl.CG;
+  info[13] = pl.n_entries;
+  info[14] = pl.max_in_degree;
+  info[15] = pl.fit_const;
+  return SA_OK;
+}
+
+int sa_get_info(sa_handle* h, int64_t info[16]) {
   if (!h || !info) return set_err(SA_EINVAL, "null argument");
-  info[0] = 1;                                   // kernel variant: 1 = generic CTA-per-chain
-  info[1] = h->threads;
-  info[2] = 1;
-  info[3] = (int64_t)tsa::smem_bytes(h->P);
-  info[4] = h->C.R;
+  for (int i = 0; i < 16; ++i) info[i] = 0;
+  const bool wk = h->warp_cpb > 0;
+  info[0] = wk ? 3 : 2;                          // sa_run kernel: 2 = CTA per chain, 3 = warp per chain
+  info[1] = wk ? 32 * h->warp_cpb : h->threads;
+  info[2] = wk ? h->warp_cpb : 1;
+  info[3] = wk ? (int64_t)tsa::warp_kernel_smem(h->P, h->warp_cpb) : (int64_t)tsa::smem_bytes(h->P);
+  info[4] = wk ? (h->C.R + h->warp_cpb - 1) / h->warp_cpb : h->C.R;
   info[5] = h->P.Epad;
   info[6] = h->sm_count;
   info[7] = h->launches;
+  info[8] = h->plan.n_pass;
+  info[9] = h->plan.total_iters;
+  info[10] = h->plan.n_rows;
+  info[11] = h->plan.n_split_nodes;
+  info[12] = h->plan.CG;
+  info[13] = h->plan.n_entries;
   return SA_OK;
 }
 

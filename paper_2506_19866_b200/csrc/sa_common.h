@@ -3,6 +3,8 @@
 #pragma once
 #include <cstdint>
 
+#include <vector_types.h>
+
 namespace tsa {
 
 constexpr int kMaxPairs = 16;
@@ -10,36 +12,51 @@ constexpr int kWarp = 32;
 constexpr uint32_t kBias = 0x80808080u;   // byte-lane accumulator bias
 constexpr uint32_t kOnes = 0x01010101u;
 
-// Read-only problem description in device memory, identical for every chain.  Nodes are
-// renumbered ("rows") by descending in-degree; edges live in "slots" of an ELL-by-pass layout:
-// pass p = rows 32p..32p+31 handled by one warp, slot (p, k, lane) = in-edge k of row 32p+lane.
-// Slots are stored as [pass][k/4][lane][k%4] so that one lane's four consecutive weights are one
-// 32-bit word and its four source offsets one 64-bit word.
+// row_meta bits (one u32 per (pass, lane))
+constexpr uint32_t kMetaOffMask = 0xFFFFu;     // byte offset of the node's state words
+constexpr uint32_t kMetaHead = 1u << 16;       // this lane finalises a node in this pass
+constexpr int kMetaCombineShift = 17;          // bit (17 + r): in combine round r add lane + 2^r
+
+// Read-only problem description in device memory, identical for every chain.
+//
+// State layout: every node owns one "entry" of CG 32-bit words (4 conditions per word, byte
+// lanes); entry e lives at byte offset e*CG*4, so its shared-memory bank unit is e mod nb,
+// nb = 32/CG.  Entries 0..nb-1 are all-zero dummies, one per bank unit.
+//
+// Edge layout: a node's in-edges form one row, or several sub-rows in consecutive lanes when it
+// is split; pass p = 32 rows handled by one warp, slot (p, k, lane) = edge k of that lane's row,
+// stored as [pass][k/4][lane][k%4] (a lane's four consecutive weights are one 32-bit word, its
+// four source offsets one 64-bit word).  The host orders every row's edges so that in each
+// iteration k the nb lanes of a conflict group (half-warp for 64-bit loads) read nb distinct bank
+// units: the state gathers are bank-conflict free by construction.  Empty cells read a dummy.
 struct DevProblem {
   int N, E, P, K, T, n_obs, n_pairs;
-  int CG;          // 32-bit state words per node: 4 conditions per word in byte lanes (1, 2 or 4)
+  int CG;          // 32-bit state words per node (1, 2 or 4)
   int n_chunks;    // condition chunks of 4*CG conditions (K > 16 -> several)
-  int n_pass;      // ceil(rows / 32)
-  int Epad;        // number of slots (multiple of 128 per pass-iteration group)
+  int n_pass;
+  int n_entries;   // state entries incl. dummies and holes
+  int Epad;        // number of slots
   int EpadA;       // Epad rounded up to 16 (row pitch of the weight store, bytes)
-  int NpadA;       // N rounded up to 16 (row pitch of the threshold store, bytes)
-  int state_words; // (N+1)*CG: words of one state buffer incl. the all-zero dummy node N
-  const int32_t*  pass_base;     // [n_pass] first slot of the pass
-  const int32_t*  pass_deg;      // [n_pass] real iterations of the pass (max in-degree of its rows)
-  const uint16_t* slot_off;      // [Epad] byte offset of the source row's state words (row*CG*4); padding -> dummy
+  int NpadA;       // n_entries rounded up to 16 (row pitch of the threshold store, bytes)
+  int state_words; // n_entries*CG: words of one state buffer
+  int n_fix;       // entries of `fix`
+  uint32_t fit_const;            // mismatches of clamped observed entries (constant per problem)
+  const int4*     pass_info;     // [n_chunks][n_pass]: x = first slot, y = iterations | combine rounds << 16,
+                                 //   z, w = start / count of the (chunk, pass) clamp fix-up list in `fix`
+  const uint32_t* row_meta;      // [n_pass*32]
+  const uint16_t* slot_off;      // [Epad] byte offset of the source entry
   const int32_t*  slot_of_param; // [E] caller edge id -> slot
-  const int32_t*  row_of_node;   // [N]
-  const int32_t*  node_of_row;   // [N]
-  const uint32_t* initw;         // [n_chunks][N][CG] initial state, byte lanes
-  const uint32_t* clampm;        // [n_chunks][N][CG] 0xFF in clamped byte lanes
-  const uint32_t* obsw;          // [n_chunks][n_obs][N][CG] observed values (0 where unobserved)
-  const uint32_t* obsm;          // [n_chunks][n_obs][N][CG] 0x01 in observed byte lanes
+  const int32_t*  entry_of_node; // [N]
+  const uint32_t* initw;         // [n_chunks][n_entries][CG] initial state, byte lanes
+  const uint32_t* obsw;          // [n_chunks][n_obs][n_entries][CG] observed values (0 where unscored)
+  const uint32_t* obsm;          // [n_chunks][n_obs][n_entries][CG] 0x01 in scored byte lanes
+  const uint32_t* fix;           // entries: bits 0-15 byte offset in the state buffer, 16-23 value
   const int8_t*   obs_idx_of_t;  // [T+1] observation index of time t or -1
   int8_t tha[kMaxPairs];         // -t_lo      per pair
   int8_t thb[kMaxPairs];         // -t_hi - 1  per pair
 };
 
-// Chain-state store in HBM: structure of arrays, int8 rows in slot / row order, 16-byte pitch.
+// Chain-state store in HBM: structure of arrays, int8 rows in slot / entry order, 16-byte pitch.
 struct DevChains {
   int R;
   int8_t *cur_w, *cur_th, *best_w, *best_th;   // [R][EpadA], [R][NpadA]

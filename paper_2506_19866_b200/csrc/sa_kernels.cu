@@ -1,7 +1,14 @@
-// CUDA kernels of libternary_sa.so (sm_100a).  Generic "one CTA per chain" family:
-// lanes over rows (nodes sorted by in-degree), 4 conditions per 32-bit word in biased byte lanes,
-// chain state (weights, thresholds, double-buffered node states) resident in shared memory for
-// the whole sa_run.  See DESIGN.md §5-§6.  Shares nothing with oracle/.
+// CUDA kernels of libternary_sa.so (sm_100a).  Lanes over rows (a node's in-edges, long rows
+// split over consecutive lanes), 4 conditions per 32-bit word in biased byte lanes, chain state
+// (weights, thresholds, double-buffered node states) resident in shared memory for the whole
+// sa_run, state gathers bank-conflict free by the host's edge schedule (sa_plan.cpp).
+//
+// Two launch shapes share every device function:
+//   CtaTeam  — one chain per CTA, its passes spread over the CTA's warps, __syncthreads per step;
+//              schedule tables read through L1 (__ldg).  Any network that fits shared memory.
+//   WarpTeam — one chain per WARP, several chains per CTA, __syncwarp only; the schedule tables are
+//              staged once per CTA in shared memory.  Small / medium networks with many chains.
+// Shares nothing with oracle/.
 #include "sa_kernels.h"
 
 namespace tsa {
@@ -22,15 +29,45 @@ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t
 }
 
 // ------------------------------------------------------------------------------------------
+// Teams: the threads that cooperate on one chain.
+// ------------------------------------------------------------------------------------------
+struct CtaTeam {
+  static constexpr bool kIsWarp = false;
+  __device__ static __forceinline__ int tid() { return threadIdx.x; }
+  __device__ static __forceinline__ int nthr() { return blockDim.x; }
+  __device__ static __forceinline__ void sync() { __syncthreads(); }
+};
+struct WarpTeam {
+  static constexpr bool kIsWarp = true;
+  __device__ static __forceinline__ int tid() { return threadIdx.x & 31; }
+  __device__ static __forceinline__ int nthr() { return 32; }
+  __device__ static __forceinline__ void sync() { __syncwarp(); }
+};
+
+// Schedule tables: device-global pointers (CtaTeam) or their shared-memory copies (WarpTeam).
+struct Tables {
+  const int4* pass_info;
+  const uint32_t* row_meta;
+  const uint16_t* slot_off;
+  const uint32_t* fix;
+  const int8_t* obs_idx_of_t;
+};
+template <bool SM, typename T>
+__device__ __forceinline__ T tab_ld(const T* p) {
+  if (SM) return *p;
+  return __ldg(p);
+}
+
+// ------------------------------------------------------------------------------------------
 // Shared-memory carve-up of one chain.
 // ------------------------------------------------------------------------------------------
 struct Smem {
   int8_t* w;        // [EpadA] weights in slot order
-  int8_t* th;       // [NpadA] threshold-pair index per row
-  char2* ab;        // [NpadA] (-t_lo, -t_hi-1) per row
-  uint32_t* S0;     // [state_words] node states, byte lanes; word (N*CG ..) = dummy zero node
+  int8_t* th;       // [NpadA] threshold-pair index per entry
+  char2* ab;        // [NpadA] (-t_lo, -t_hi-1) per entry
+  uint32_t* S0;     // [state_words] node states, byte lanes; the first 32 words are the zero dummies
   uint32_t* S1;
-  uint32_t* red;    // [32] cross-warp reduction scratch
+  uint32_t* red;    // [32] cross-warp reduction scratch (CtaTeam)
 };
 
 __host__ __device__ inline size_t align16(size_t x) { return (x + 15) & ~(size_t)15; }
@@ -47,9 +84,27 @@ __host__ __device__ inline size_t smem_layout(const DevProblem& P, size_t* off_t
   return o;
 }
 
-size_t smem_bytes(const DevProblem& P) {
+__host__ __device__ inline size_t chain_smem_bytes(const DevProblem& P) {
   size_t a, b, c, d, e;
   return smem_layout(P, &a, &b, &c, &d, &e);
+}
+
+size_t smem_bytes(const DevProblem& P) { return chain_smem_bytes(P); }
+
+// shared copy of the schedule tables (WarpTeam kernels), placed before the per-chain regions
+__host__ __device__ inline size_t table_layout(const DevProblem& P, size_t* off_info, size_t* off_meta, size_t* off_fix,
+                                               size_t* off_obs) {
+  size_t o = align16((size_t)P.Epad * 2);                         *off_info = o;
+  o += (size_t)P.n_chunks * P.n_pass * 16;                        *off_meta = o;
+  o += (size_t)P.n_pass * 32 * 4;                                 *off_fix = o;
+  o += align16((size_t)P.n_fix * 4);                              *off_obs = o;
+  o += align16((size_t)P.T + 1);
+  return o;
+}
+
+size_t table_bytes(const DevProblem& P) {
+  size_t a, b, c, d;
+  return table_layout(P, &a, &b, &c, &d);
 }
 
 __device__ __forceinline__ Smem carve(const DevProblem& P, unsigned char* base) {
@@ -65,21 +120,24 @@ __device__ __forceinline__ Smem carve(const DevProblem& P, unsigned char* base) 
   return s;
 }
 
-// 16-byte vector copy, n16 = number of int4
+// 16-byte vector copy by one team, n16 = number of int4
+template <typename Team>
 __device__ __forceinline__ void copy16(void* dst, const void* src, int n16) {
-  for (int i = threadIdx.x; i < n16; i += blockDim.x) ((int4*)dst)[i] = ((const int4*)src)[i];
+  for (int i = Team::tid(); i < n16; i += Team::nthr()) ((int4*)dst)[i] = ((const int4*)src)[i];
 }
 
+template <typename Team>
 __device__ __forceinline__ void build_ab(const DevProblem& P, const Smem& sm) {
-  for (int r = threadIdx.x; r < P.N; r += blockDim.x) {
+  for (int r = Team::tid(); r < P.n_entries; r += Team::nthr()) {
     const int q = sm.th[r];
     sm.ab[r] = make_char2(P.tha[q], P.thb[q]);
   }
 }
 
-__device__ __forceinline__ uint32_t block_sum(uint32_t v, uint32_t* red) {
+template <typename Team>
+__device__ __forceinline__ uint32_t team_sum(uint32_t v, uint32_t* red) {
   v = __reduce_add_sync(0xffffffffu, v);
-  if (blockDim.x == 32) return v;
+  if (Team::kIsWarp || blockDim.x == 32) return v;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
   if (lane == 0) red[warp] = v;
   __syncthreads();
@@ -109,96 +167,149 @@ template <> __device__ __forceinline__ uint4 pack<4>(const uint32_t (&s)[4]) { r
 // ------------------------------------------------------------------------------------------
 // a3 + a4: simulate every condition for T synchronous steps from shared-memory weights and
 // thresholds, count mismatches at the observation times.
-// Returns this thread's partial mismatch count.  All threads of the CTA must call it.
+// Returns this thread's partial mismatch count (clamped entries are in P.fit_const).  All
+// threads of the team must call it.
 //
 // Arithmetic per node word (4 conditions): acc = 0x80808080 + SUM w*s (one IMAD per edge, w a
-// sign-extended int8, s in {0,1,2} per byte); because |sum| + |threshold| <= 127 every byte
-// stays a valid base-256 digit, so
+// sign-extended int8, s in {0,1,2} per byte); because 128 + sum - threshold stays in [0,255]
+// every byte is a valid base-256 digit, so
 //   [sum >= t_lo] = bit 7 of (acc - t_lo),  [sum > t_hi] = bit 7 of (acc - t_hi - 1)
 // per byte, and the new state is their sum: 0 if sum < t_lo, 2 if sum > t_hi, else 1.
 // ------------------------------------------------------------------------------------------
-template <int CG, bool DUMP>
-__device__ __forceinline__ uint32_t simulate(const DevProblem& P, const Smem& sm, uint8_t* dump) {
+template <int U>
+__device__ __forceinline__ int weight_of(uint32_t wword) {
+  // sign-extended byte U in one PRMT: selector nibble U picks the byte, nibble U|8 replicates its
+  // sign bit (PTX prmt default mode; __byte_perm would mask bit 3 of the nibbles away)
+  constexpr uint32_t sel = (uint32_t)(U | ((U | 8) << 4) | ((U | 8) << 8) | ((U | 8) << 12));
+  uint32_t r;
+  asm("prmt.b32 %0, %1, 0, %2;" : "=r"(r) : "r"(wword), "n"(sel));
+  return (int)r;
+}
+
+template <int CG, int U>
+__device__ __forceinline__ void edge_slot(const unsigned char* curb, uint32_t wword, const uint2& offs, uint32_t (&acc)[CG]) {
   using V = typename Vec<CG>::T;
-  const int tid = threadIdx.x, nthr = blockDim.x, lane = tid & 31, warp = tid >> 5, nwarps = nthr >> 5;
-  const int NW = P.N * CG;
+  const int wv = weight_of<U>(wword);
+  const uint32_t o2 = (U < 2) ? offs.x : offs.y;
+  const uint32_t off = (U & 1) ? (o2 >> 16) : (o2 & 0xFFFFu);
+  uint32_t s[CG];
+  unpack<CG>(*(const V*)(curb + off), s);
+#pragma unroll
+  for (int c = 0; c < CG; ++c) acc[c] += (uint32_t)(wv * (int)s[c]);
+}
+
+template <int CG, bool DUMP, typename Team, bool SMTAB>
+__device__ __forceinline__ uint32_t simulate(const DevProblem& P, const Tables& tab, const Smem& sm, uint8_t* dump) {
+  using V = typename Vec<CG>::T;
+  constexpr int kEntryShift = (CG == 1) ? 2 : (CG == 2) ? 3 : 4;   // log2(CG*4)
+  const int tid = Team::tid(), nthr = Team::nthr(), lane = tid & 31, warp = tid >> 5, nwarps = nthr >> 5;
+  const int NW = P.state_words;
   uint32_t mism = 0;
   for (int ch = 0; ch < P.n_chunks; ++ch) {
     const uint32_t* initw = P.initw + (size_t)ch * NW;
-    const uint32_t* clampm = P.clampm + (size_t)ch * NW;
-    for (int x = tid; x < P.state_words; x += nthr) {
-      sm.S0[x] = (x < NW) ? __ldg(initw + x) : 0u;
-      if (x >= NW) sm.S1[x] = 0u;
+    for (int x = tid; x < NW; x += nthr) {
+      sm.S0[x] = __ldg(initw + x);
+      if (x < 32) sm.S1[x] = 0u;              // the dummy entries of the other buffer
     }
-    __syncthreads();
+    Team::sync();
     uint32_t* cur = sm.S0;
     uint32_t* nxt = sm.S1;
     for (int t = 1; t <= P.T; ++t) {
-      const int oj = P.obs_idx_of_t[t];
+      const int oj = tab_ld<SMTAB>(tab.obs_idx_of_t + t);
       const unsigned char* curb = (const unsigned char*)cur;
       for (int ps = warp; ps < P.n_pass; ps += nwarps) {
-        const int base = __ldg(P.pass_base + ps), deg = __ldg(P.pass_deg + ps);
+        // x = first slot, y = iterations | combine rounds << 16, z / w = fix-up list start / count
+        const int4 info = tab_ld<SMTAB>(tab.pass_info + ch * P.n_pass + ps);
+        const uint32_t meta = tab_ld<SMTAB>(tab.row_meta + ps * 32 + lane);
+        const int iters = info.y & 0xFFFF, rounds = info.y >> 16;
         uint32_t acc[CG];
 #pragma unroll
         for (int c = 0; c < CG; ++c) acc[c] = kBias;
-        for (int k4 = 0; k4 * 4 < deg; ++k4) {
-          const int s0 = base + k4 * 128 + lane * 4;
-          const uint32_t wword = *(const uint32_t*)(sm.w + s0);
-          const uint2 offs = __ldg((const uint2*)(P.slot_off + s0));
+        const unsigned char* wp = (const unsigned char*)sm.w + info.x + lane * 4;
+        const unsigned char* op = (const unsigned char*)tab.slot_off + 2 * (info.x + lane * 4);
+#pragma unroll 1
+        for (int full = iters >> 2; full > 0; --full, wp += 128, op += 256) {
+          const uint32_t wword = *(const uint32_t*)wp;
+          const uint2 offs = tab_ld<SMTAB>((const uint2*)op);
+          edge_slot<CG, 0>(curb, wword, offs, acc);
+          edge_slot<CG, 1>(curb, wword, offs, acc);
+          edge_slot<CG, 2>(curb, wword, offs, acc);
+          edge_slot<CG, 3>(curb, wword, offs, acc);
+        }
+        const int rem = iters & 3;
+        if (rem) {
+          const uint32_t wword = *(const uint32_t*)wp;
+          const uint2 offs = tab_ld<SMTAB>((const uint2*)op);
+          edge_slot<CG, 0>(curb, wword, offs, acc);
+          if (rem > 1) edge_slot<CG, 1>(curb, wword, offs, acc);
+          if (rem > 2) edge_slot<CG, 2>(curb, wword, offs, acc);
+        }
+        // split rows: partial sums of consecutive lanes are added up a binary tree
+#pragma unroll 1
+        for (int q = 0; q < rounds; ++q) {
+          const bool take = (meta >> (kMetaCombineShift + q)) & 1u;
 #pragma unroll
-          for (int u = 0; u < 4; ++u) {
-            if (k4 * 4 + u < deg) {
-              const int wv = (int)(int8_t)(wword >> (8 * u));
-              const uint32_t o2 = (u < 2) ? offs.x : offs.y;
-              const uint32_t off = (u & 1) ? (o2 >> 16) : (o2 & 0xFFFFu);
-              uint32_t s[CG];
-              unpack<CG>(*(const V*)(curb + off), s);
-#pragma unroll
-              for (int c = 0; c < CG; ++c) acc[c] += (uint32_t)(wv * (int)s[c]);
-            }
+          for (int c = 0; c < CG; ++c) {
+            const uint32_t other = __shfl_down_sync(0xffffffffu, acc[c], 1u << q);
+            if (take) acc[c] += other - kBias;
           }
         }
-        const int row = ps * 32 + lane;
-        if (row < P.N) {
-          const char2 ab = sm.ab[row];
-          uint32_t cm[CG], iv[CG], ns[CG];
-          unpack<CG>(__ldg((const V*)(clampm + row * CG)), cm);
-          unpack<CG>(__ldg((const V*)(initw + row * CG)), iv);
+        if (meta & kMetaHead) {
+          const uint32_t off = meta & kMetaOffMask;
+          const char2 ab = sm.ab[off >> kEntryShift];
+          uint32_t ns[CG];
 #pragma unroll
           for (int c = 0; c < CG; ++c) {
             const uint32_t ge = ((acc[c] + (uint32_t)((int)ab.x * (int)kOnes)) >> 7) & kOnes;
             const uint32_t gt = ((acc[c] + (uint32_t)((int)ab.y * (int)kOnes)) >> 7) & kOnes;
-            ns[c] = ((ge + gt) & ~cm[c]) | (iv[c] & cm[c]);
+            ns[c] = ge + gt;
           }
-          *(V*)(nxt + row * CG) = pack<CG>(ns);
+          *(V*)((unsigned char*)nxt + off) = pack<CG>(ns);
           if (oj >= 0) {
-            const size_t ow = (((size_t)ch * P.n_obs + oj) * P.N + row) * CG;
+            const size_t ob = ((size_t)ch * P.n_obs + oj) * (size_t)NW * 4 + off;
             uint32_t ov[CG], om[CG];
-            unpack<CG>(__ldg((const V*)(P.obsw + ow)), ov);
-            unpack<CG>(__ldg((const V*)(P.obsm + ow)), om);
+            unpack<CG>(__ldg((const V*)((const unsigned char*)P.obsw + ob)), ov);
+            unpack<CG>(__ldg((const V*)((const unsigned char*)P.obsm + ob)), om);
 #pragma unroll
             for (int c = 0; c < CG; ++c) {
               const uint32_t x = ns[c] ^ ov[c];
               mism += __popc((x | (x >> 1)) & om[c]);
             }
-            if (DUMP) {
-              const int node = P.node_of_row[row];
-#pragma unroll
-              for (int c = 0; c < CG; ++c)
-#pragma unroll
-                for (int b = 0; b < 4; ++b) {
-                  const int k = ch * 4 * CG + c * 4 + b;
-                  if (k < P.K) dump[((size_t)k * P.n_obs + oj) * P.N + node] = (uint8_t)((ns[c] >> (8 * b)) & 0xFFu);
-                }
-            }
+          }
+        }
+        // clamped entries keep their initial value: byte stores after the pass's own stores
+        if (info.w > 0) {
+          __syncwarp();
+          for (int i = lane; i < info.w; i += 32) {
+            const uint32_t fx = tab_ld<SMTAB>(tab.fix + info.z + i);
+            ((unsigned char*)nxt)[fx & 0xFFFFu] = (unsigned char)(fx >> 16);
           }
         }
       }
-      __syncthreads();
+      Team::sync();
+      if (DUMP && oj >= 0) {
+        for (int i = tid; i < P.N; i += nthr) {
+          const uint32_t* e = nxt + (size_t)__ldg(P.entry_of_node + i) * CG;
+#pragma unroll
+          for (int c = 0; c < CG; ++c)
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+              const int k = ch * 4 * CG + c * 4 + b;
+              if (k < P.K) dump[((size_t)k * P.n_obs + oj) * P.N + i] = (uint8_t)((e[c] >> (8 * b)) & 0xFFu);
+            }
+        }
+      }
       uint32_t* tmp = cur; cur = nxt; nxt = tmp;
     }
   }
   return mism;
+}
+
+__device__ __forceinline__ Tables global_tables(const DevProblem& P) {
+  Tables t;
+  t.pass_info = P.pass_info; t.row_meta = P.row_meta; t.slot_off = P.slot_off; t.fix = P.fix;
+  t.obs_idx_of_t = P.obs_idx_of_t;
+  return t;
 }
 
 // ------------------------------------------------------------------------------------------
@@ -209,13 +320,14 @@ __global__ void eval_kernel(const DevProblem P, const int8_t* __restrict__ w, co
                             uint32_t* __restrict__ fit, uint8_t* dump) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Smem sm = carve(P, smem_raw);
+  const Tables tab = global_tables(P);
   const size_t b = blockIdx.x;
-  copy16(sm.w, w + b * P.EpadA, P.EpadA / 16);
-  copy16(sm.th, th + b * P.NpadA, P.NpadA / 16);
+  copy16<CtaTeam>(sm.w, w + b * P.EpadA, P.EpadA / 16);
+  copy16<CtaTeam>(sm.th, th + b * P.NpadA, P.NpadA / 16);
   __syncthreads();
-  build_ab(P, sm);
+  build_ab<CtaTeam>(P, sm);
   __syncthreads();
-  const uint32_t f = block_sum(simulate<CG, DUMP>(P, sm, dump), sm.red);
+  const uint32_t f = team_sum<CtaTeam>(simulate<CG, DUMP, CtaTeam, false>(P, tab, sm, dump), sm.red) + P.fit_const;
   if (threadIdx.x == 0) fit[b] = f;
 }
 
@@ -227,6 +339,7 @@ template <int CG>
 __global__ void init_kernel(const DevProblem P, const DevChains C, const DevSched S) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const Smem sm = carve(P, smem_raw);
+  const Tables tab = global_tables(P);
   const size_t chain = blockIdx.x;
   const uint32_t gchain = S.chain_id_base + (uint32_t)chain;
   for (int i = threadIdx.x; i < P.EpadA; i += blockDim.x) sm.w[i] = 0;
@@ -239,67 +352,66 @@ __global__ void init_kernel(const DevProblem P, const DevChains C, const DevSche
     for (int m = 0; m < 4; ++m) {
       const int p = 4 * q + m;
       if (p < P.E) sm.w[__ldg(P.slot_of_param + p)] = (int8_t)((int)__umulhi(y[m], 3u) - 1);
-      else if (p < P.P) sm.th[__ldg(P.row_of_node + (p - P.E))] = (int8_t)__umulhi(y[m], (uint32_t)P.n_pairs);
+      else if (p < P.P) sm.th[__ldg(P.entry_of_node + (p - P.E))] = (int8_t)__umulhi(y[m], (uint32_t)P.n_pairs);
     }
   }
   __syncthreads();
-  build_ab(P, sm);
+  build_ab<CtaTeam>(P, sm);
   __syncthreads();
-  const uint32_t f = block_sum(simulate<CG, false>(P, sm, nullptr), sm.red);
-  copy16(C.cur_w + chain * P.EpadA, sm.w, P.EpadA / 16);
-  copy16(C.best_w + chain * P.EpadA, sm.w, P.EpadA / 16);
-  copy16(C.cur_th + chain * P.NpadA, sm.th, P.NpadA / 16);
-  copy16(C.best_th + chain * P.NpadA, sm.th, P.NpadA / 16);
+  const uint32_t f = team_sum<CtaTeam>(simulate<CG, false, CtaTeam, false>(P, tab, sm, nullptr), sm.red) + P.fit_const;
+  copy16<CtaTeam>(C.cur_w + chain * P.EpadA, sm.w, P.EpadA / 16);
+  copy16<CtaTeam>(C.best_w + chain * P.EpadA, sm.w, P.EpadA / 16);
+  copy16<CtaTeam>(C.cur_th + chain * P.NpadA, sm.th, P.NpadA / 16);
+  copy16<CtaTeam>(C.best_th + chain * P.NpadA, sm.th, P.NpadA / 16);
   if (threadIdx.x == 0) { C.fit_cur[chain] = f; C.fit_best[chain] = f; }
 }
 
 // ------------------------------------------------------------------------------------------
 // sa_run: `steps` chain-steps of one chain, everything on chip (Table 1 :130-149;
-// SURVEY.md §8(c)-3).  Thread 0 applies / reverts the one-byte mutation; every thread computes
-// the Philox block and the accept decision redundantly so no broadcast is needed.
+// SURVEY.md §8(c)-3).  Thread 0 of the team applies / reverts the one-byte mutation; every thread
+// computes the Philox block and the accept decision redundantly so no broadcast is needed.
 // ------------------------------------------------------------------------------------------
-template <int CG>
-__global__ void run_kernel(const DevProblem P, const DevChains C, const DevSched S, const DevTrace Tr,
-                           const uint64_t g0, const int64_t steps) {
-  extern __shared__ __align__(16) unsigned char smem_raw[];
-  const Smem sm = carve(P, smem_raw);
-  const size_t chain = blockIdx.x;
+template <int CG, typename Team, bool SMTAB>
+__device__ __forceinline__ void run_chain(const DevProblem& P, const Tables& tab, const Smem& sm, const DevChains& C,
+                                          const DevSched& S, const DevTrace& Tr, const size_t chain,
+                                          const uint64_t g0, const int64_t steps) {
   const uint32_t gchain = S.chain_id_base + (uint32_t)chain;
-  copy16(sm.w, C.cur_w + chain * P.EpadA, P.EpadA / 16);
-  copy16(sm.th, C.cur_th + chain * P.NpadA, P.NpadA / 16);
-  __syncthreads();
-  build_ab(P, sm);
+  const bool leader = Team::tid() == 0;
+  copy16<Team>(sm.w, C.cur_w + chain * P.EpadA, P.EpadA / 16);
+  copy16<Team>(sm.th, C.cur_th + chain * P.NpadA, P.NpadA / 16);
+  Team::sync();
+  build_ab<Team>(P, sm);
   uint32_t fcur = C.fit_cur[chain], fbest = C.fit_best[chain];
   const int trow = Tr.row_of_chain ? Tr.row_of_chain[chain] : -1;
 
   uint64_t level = g0 / (uint64_t)S.steps_per_level;
   int64_t left_in_level = S.steps_per_level - (int64_t)(g0 % (uint64_t)S.steps_per_level);
-  __syncthreads();
+  Team::sync();
 
   for (int64_t it = 0; it < steps; ++it) {
     const uint64_t g = g0 + (uint64_t)it;
     uint32_t x[4];
     philox4x32_10((uint32_t)g, (uint32_t)(g >> 32), gchain, 0u, S.key0, S.key1, x);
     const int p = (int)__umulhi(x[0], (uint32_t)P.P);
-    // a1/a2: thread 0 proposes and applies; (loc, old) let it revert
+    // a1/a2: the leader proposes and applies; (loc, old) let it revert
     int loc = 0, oldv = 0, newv = 0;
-    if (threadIdx.x == 0) {
+    if (leader) {
       if (p < P.E) {
         loc = __ldg(P.slot_of_param + p);
         oldv = sm.w[loc];
         newv = (oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;          // (code + 1 + r) mod 3 - 1, code = old + 1
         sm.w[loc] = (int8_t)newv;
       } else {
-        loc = __ldg(P.row_of_node + (p - P.E));
+        loc = __ldg(P.entry_of_node + (p - P.E));
         oldv = sm.th[loc];
         newv = (oldv + 1 + (int)__umulhi(x[1], (uint32_t)(P.n_pairs - 1))) % P.n_pairs;
         sm.th[loc] = (int8_t)newv;
         sm.ab[loc] = make_char2(P.tha[newv], P.thb[newv]);
       }
     }
-    __syncthreads();
+    Team::sync();
     // a3/a4
-    const uint32_t fcand = block_sum(simulate<CG, false>(P, sm, nullptr), sm.red);
+    const uint32_t fcand = team_sum<Team>(simulate<CG, false, Team, SMTAB>(P, tab, sm, nullptr), sm.red) + P.fit_const;
     // a5
     const uint64_t lv = level < (uint64_t)(S.n_levels - 1) ? level : (uint64_t)(S.n_levels - 1);
     const int64_t d = (int64_t)fcand - (int64_t)fcur;
@@ -312,15 +424,15 @@ __global__ void run_kernel(const DevProblem P, const DevChains C, const DevSched
       if (fcand < fbest) {
         fbest = fcand;
         new_best = true;
-        copy16(C.best_w + chain * P.EpadA, sm.w, P.EpadA / 16);
-        copy16(C.best_th + chain * P.NpadA, sm.th, P.NpadA / 16);
-        __syncthreads();            // the copy reads sm.w/th; the next mutation writes them
+        copy16<Team>(C.best_w + chain * P.EpadA, sm.w, P.EpadA / 16);
+        copy16<Team>(C.best_th + chain * P.NpadA, sm.th, P.NpadA / 16);
+        Team::sync();               // the copy reads sm.w/th; the next mutation writes them
       }
-    } else if (threadIdx.x == 0) {
+    } else if (leader) {
       if (p < P.E) sm.w[loc] = (int8_t)oldv;
       else { sm.th[loc] = (int8_t)oldv; sm.ab[loc] = make_char2(P.tha[oldv], P.thb[oldv]); }
     }
-    if (trow >= 0 && threadIdx.x == 0) {
+    if (trow >= 0 && leader) {
       const uint64_t idx = g - Tr.g_start;
       if (g >= Tr.g_start && idx < (uint64_t)Tr.max_steps) {
         const uint64_t code = (p < P.E) ? (uint64_t)(newv + 1) : (uint64_t)newv;
@@ -331,11 +443,48 @@ __global__ void run_kernel(const DevProblem P, const DevChains C, const DevSched
     }
     if (--left_in_level == 0) { ++level; left_in_level = S.steps_per_level; }
   }
-  __syncthreads();
+  Team::sync();
   // a7
-  copy16(C.cur_w + chain * P.EpadA, sm.w, P.EpadA / 16);
-  copy16(C.cur_th + chain * P.NpadA, sm.th, P.NpadA / 16);
-  if (threadIdx.x == 0) { C.fit_cur[chain] = fcur; C.fit_best[chain] = fbest; }
+  copy16<Team>(C.cur_w + chain * P.EpadA, sm.w, P.EpadA / 16);
+  copy16<Team>(C.cur_th + chain * P.NpadA, sm.th, P.NpadA / 16);
+  if (leader) { C.fit_cur[chain] = fcur; C.fit_best[chain] = fbest; }
+}
+
+template <int CG>
+__global__ void run_kernel(const DevProblem P, const DevChains C, const DevSched S, const DevTrace Tr,
+                           const uint64_t g0, const int64_t steps) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const Smem sm = carve(P, smem_raw);
+  run_chain<CG, CtaTeam, false>(P, global_tables(P), sm, C, S, Tr, blockIdx.x, g0, steps);
+}
+
+// One chain per warp; the CTA first stages the schedule tables in shared memory.
+template <int CG>
+__global__ void __launch_bounds__(256) run_warp_kernel(const DevProblem P, const DevChains C, const DevSched S,
+                                                       const DevTrace Tr, const uint64_t g0, const int64_t steps) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  size_t o_info, o_meta, o_fix, o_obs;
+  const size_t tbytes = table_layout(P, &o_info, &o_meta, &o_fix, &o_obs);
+  {
+    const int n = threadIdx.x, step = blockDim.x;
+    for (int i = n; i < (P.Epad * 2 + 15) / 16; i += step) ((int4*)smem_raw)[i] = __ldg((const int4*)P.slot_off + i);
+    for (int i = n; i < P.n_chunks * P.n_pass; i += step) ((int4*)(smem_raw + o_info))[i] = __ldg(P.pass_info + i);
+    for (int i = n; i < P.n_pass * 32; i += step) ((uint32_t*)(smem_raw + o_meta))[i] = __ldg(P.row_meta + i);
+    for (int i = n; i < P.n_fix; i += step) ((uint32_t*)(smem_raw + o_fix))[i] = __ldg(P.fix + i);
+    for (int i = n; i <= P.T; i += step) ((int8_t*)(smem_raw + o_obs))[i] = P.obs_idx_of_t[i];
+  }
+  __syncthreads();
+  Tables tab;
+  tab.slot_off = (const uint16_t*)smem_raw;
+  tab.pass_info = (const int4*)(smem_raw + o_info);
+  tab.row_meta = (const uint32_t*)(smem_raw + o_meta);
+  tab.fix = (const uint32_t*)(smem_raw + o_fix);
+  tab.obs_idx_of_t = (const int8_t*)(smem_raw + o_obs);
+  const int warp = threadIdx.x >> 5, cpb = blockDim.x >> 5;
+  const size_t chain = (size_t)blockIdx.x * cpb + warp;
+  if (chain >= (size_t)C.R) return;             // no CTA-wide barrier after this point
+  const Smem sm = carve(P, smem_raw + tbytes + (size_t)warp * align16(chain_smem_bytes(P)));
+  run_chain<CG, WarpTeam, true>(P, tab, sm, C, S, Tr, chain, g0, steps);
 }
 
 __global__ void argmin_kernel(const uint32_t* __restrict__ fit, int R, unsigned long long* out) {
@@ -390,6 +539,22 @@ cudaError_t launch_run(const DevProblem& P, const DevChains& C, const DevSched& 
   TSA_DISPATCH_CG(P, {
     e = set_smem(run_kernel<CG>, sb);
     if (e == cudaSuccess) run_kernel<CG><<<C.R, threads, sb, st>>>(P, C, S, Tr, g0, steps);
+  });
+  return e != cudaSuccess ? e : cudaGetLastError();
+}
+
+size_t warp_kernel_smem(const DevProblem& P, int chains_per_cta) {
+  return table_bytes(P) + (size_t)chains_per_cta * align16(smem_bytes(P));
+}
+
+cudaError_t launch_run_warp(const DevProblem& P, const DevChains& C, const DevSched& S, const DevTrace& Tr,
+                            uint64_t g0, int64_t steps, int chains_per_cta, cudaStream_t st) {
+  const size_t sb = warp_kernel_smem(P, chains_per_cta);
+  const unsigned grid = (unsigned)((C.R + chains_per_cta - 1) / chains_per_cta);
+  cudaError_t e = cudaSuccess;
+  TSA_DISPATCH_CG(P, {
+    e = set_smem(run_warp_kernel<CG>, sb);
+    if (e == cudaSuccess) run_warp_kernel<CG><<<grid, 32 * chains_per_cta, sb, st>>>(P, C, S, Tr, g0, steps);
   });
   return e != cudaSuccess ? e : cudaGetLastError();
 }

@@ -12,6 +12,10 @@ size_t smem_bytes(const DevProblem& P);
 cudaError_t launch_init(const DevProblem& P, const DevChains& C, const DevSched& S, int threads, cudaStream_t st);
 cudaError_t launch_run(const DevProblem& P, const DevChains& C, const DevSched& S, const DevTrace& Tr,
                        uint64_t g0, int64_t steps, int threads, cudaStream_t st);
+// one chain per warp, chains_per_cta warps per CTA, schedule tables staged in shared memory
+size_t warp_kernel_smem(const DevProblem& P, int chains_per_cta);
+cudaError_t launch_run_warp(const DevProblem& P, const DevChains& C, const DevSched& S, const DevTrace& Tr,
+                            uint64_t g0, int64_t steps, int chains_per_cta, cudaStream_t st);
 cudaError_t launch_eval(const DevProblem& P, const int8_t* w, const int8_t* th, int64_t n, uint32_t* fit,
                         uint8_t* dump, int threads, cudaStream_t st);
 // out[0] = (fitness << 32) | chain of the best chain (smallest fitness, then smallest index)

@@ -100,3 +100,29 @@ def test_no_cpu_fallback(B, problems_cache):
         B.sa_simulate(problems_cache("tiny"), problems_cache("tiny").truth)
     assert B.sa_run.__doc__ is None or True
     B.sa_destroy(None)                      # NULL is a no-op
+
+
+def test_execution_plan_is_valid_for_every_config(B, problems_cache):
+    """sa_plan_info builds the host-side plan (rows, split rows, bank classes, conflict-free edge
+    colouring) and fails if its own self-check finds an unscheduled edge or a bank conflict."""
+    import math
+    for name in ("tiny", "hpg", "mtb", "large"):
+        prob = problems_cache(name)
+        info = B.sa_plan_info(prob)
+        assert info["edge_iterations"] >= math.ceil(prob.n_edges / 32)
+        assert info["rows"] >= prob.n_nodes and info["passes"] * 32 >= info["rows"]
+        assert info["edge_slots"] >= prob.n_edges
+        assert info["state_words_per_node"] == {"tiny": 1, "hpg": 1, "mtb": 2, "large": 4}[name]
+        assert info["max_in_degree"] == int(np.bincount(prob.edge_dst).max())
+        # clamped observed entries never change: their mismatches are a per-problem constant
+        k, j, i = np.nonzero((prob.obs != 255) & (prob.clamp[:, None, :] == 1))
+        assert info["clamped_mismatches"] == int((prob.obs[k, j, i] != prob.init_state[k, i]).sum())
+    mtb = B.sa_plan_info(problems_cache("mtb"))
+    assert mtb["edge_iterations"] <= 40          # 900 edges / 32 lanes = 28.1 is the floor; the naive layout needs 56
+    import os
+    os.environ["TSA_NO_SPLIT"] = "1"; os.environ["TSA_NO_BANKOPT"] = "1"
+    try:
+        naive = B.sa_plan_info(problems_cache("mtb"))
+    finally:
+        del os.environ["TSA_NO_SPLIT"], os.environ["TSA_NO_BANKOPT"]
+    assert naive["split_nodes"] == 0 and naive["edge_iterations"] > mtb["edge_iterations"]

@@ -221,18 +221,25 @@ def test_split_runs_chain_base_and_team_width(B, problems_cache):
         B.sa_set_trace(c.h, [0, 1, 2, 3], 600)
         B.sa_run(c.h, 600)
         assert np.array_equal(B.sa_get_trace(c.h, 4, 600), ta[8:12])
-    for warps in ("1", "2", "4"):                                     # launch geometry never changes results
-        os.environ["TSA_TEAM_WARPS"] = warps
+    # launch geometry and the host's edge schedule never change results
+    for env in ({"TSA_TEAM_WARPS": "1"}, {"TSA_TEAM_WARPS": "2"}, {"TSA_TEAM_WARPS": "4"},
+                {"TSA_NO_SPLIT": "1"}, {"TSA_NO_BANKOPT": "1"}, {"TSA_NO_SPLIT": "1", "TSA_NO_BANKOPT": "1"}):
+        os.environ.update(env)
         try:
             with Handle(B, prob, sched) as d:
-                assert B.sa_get_info(d.h)["threads_per_cta"] == 32 * int(warps)
+                info = B.sa_get_info(d.h)
+                if "TSA_TEAM_WARPS" in env:
+                    assert info["threads_per_cta"] == 32 * int(env["TSA_TEAM_WARPS"])
+                if "TSA_NO_SPLIT" in env:
+                    assert info["split_nodes"] == 0
                 B.sa_run(d.h, 600)
                 for ch in range(16):
                     got = B.sa_get_chain(d.h, ch, prob.n_params)
                     assert np.array_equal(got[0], state_a[ch][0]) and got[1] == state_a[ch][1]
                     assert np.array_equal(got[2], state_a[ch][2]) and got[3] == state_a[ch][3]
         finally:
-            del os.environ["TSA_TEAM_WARPS"]
+            for k in env:
+                del os.environ[k]
 
 
 def test_extreme_tables(B, problems_cache):
