@@ -19,7 +19,9 @@ LIB_PATH = os.path.join(_HERE, "libternary_sa.so")
 SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
-           "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info")
+           "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info",
+           "sa_select_kernel", "sa_jit_check")
+SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC = 0, 1, 2
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2506_19866_b200.build` "
@@ -71,6 +73,8 @@ _lib.sa_plan_info.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c
 _lib.sa_set_stream.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_set_allocator.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_int32_peak.argtypes = [C.c_void_p]
+_lib.sa_select_kernel.argtypes = [C.c_void_p, C.c_int]
+_lib.sa_jit_check.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c_int32, C.c_void_p, C.c_char_p, C.c_size_t]
 
 
 def _check(rc: int, where: str):
@@ -221,7 +225,8 @@ def sa_get_info(h: int) -> dict:
     info = np.zeros(16, dtype=np.int64)
     _check(_lib.sa_get_info(h, info.ctypes.data), "sa_get_info")
     keys = ("variant", "threads_per_cta", "chains_per_cta", "smem_bytes", "grid", "edge_slots", "sm_count", "launches",
-            "passes", "edge_iterations", "rows", "split_nodes", "state_words_per_node", "state_entries")
+            "passes", "edge_iterations", "rows", "split_nodes", "state_words_per_node", "state_entries",
+            "static_regs", "team_warps")
     return dict(zip(keys, (int(v) for v in info)))
 
 
@@ -232,6 +237,20 @@ def sa_plan_info(prob) -> dict:
     return {"variant": int(info[0]), "edge_slots": int(info[5]), "passes": int(info[8]), "edge_iterations": int(info[9]),
             "rows": int(info[10]), "split_nodes": int(info[11]), "state_words_per_node": int(info[12]),
             "state_entries": int(info[13]), "max_in_degree": int(info[14]), "clamped_mismatches": int(info[15])}
+
+
+def sa_select_kernel(h: int, family: int) -> None:
+    _check(_lib.sa_select_kernel(h, family), "sa_select_kernel")
+
+
+def sa_jit_check(prob, n_chains: int) -> dict:
+    """Host only: plan + NVRTC compile of the statically scheduled kernel for this problem."""
+    net, obs, keep = _marshal_problem(prob, need_obs=getattr(prob, "obs", None) is not None)
+    info = np.zeros(8, dtype=np.int64)
+    log = C.create_string_buffer(16384)
+    _check(_lib.sa_jit_check(C.byref(net), C.byref(obs), n_chains, info.ctypes.data, log, len(log)), "sa_jit_check")
+    return {"applies": bool(info[0]), "team_warps": int(info[1]), "tiers": int(info[2]), "lane_slots": int(info[3]),
+            "cubin_bytes": int(info[4]), "smem_bytes": int(info[5]), "log": log.value.decode(errors="replace")}
 
 
 def sa_int32_peak() -> dict:

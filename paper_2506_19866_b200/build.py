@@ -11,7 +11,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libternary_sa.so")
-SOURCES = ["sa_api.cu", "sa_kernels.cu", "sa_peak.cu", "sa_plan.cpp"]
+SOURCES = ["sa_api.cu", "sa_kernels.cu", "sa_peak.cu", "sa_plan.cpp", "sa_jit.cpp", "sa_static_aot.cu"]
+EMBED = os.path.join(CSRC, "sa_static_source.inc")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "--use_fast_math"]
 
@@ -35,12 +36,30 @@ def stale() -> bool:
     return any(os.path.getmtime(d) > t for d in _deps())
 
 
+def embed_static_source() -> None:
+    """sa_static_source.inc = params header + kernel source as one C++ raw string literal: the
+    text NVRTC compiles at run time (sa_jit.cpp)."""
+    parts = []
+    for name in ("sa_static_params.h", "sa_static_kernel.cu"):
+        with open(os.path.join(CSRC, name)) as f:
+            parts.append(f.read())
+    text = 'R"TSASRC(' + "\n".join(parts) + ')TSASRC"\n'
+    old = None
+    if os.path.exists(EMBED):
+        with open(EMBED) as f:
+            old = f.read()
+    if old != text:
+        with open(EMBED, "w") as f:
+            f.write(text)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     if not force and not stale():
         return LIB
+    embed_static_source()
     tmp = LIB + ".tmp.%d" % os.getpid()
     cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-shared", "-o", tmp]
-    cmd += [os.path.join(CSRC, s) for s in SOURCES]
+    cmd += [os.path.join(CSRC, s) for s in SOURCES] + ["-ldl"]
     if verbose:
         print(" ".join(cmd))
     subprocess.check_call(cmd)

@@ -11,6 +11,7 @@
 
 #include "../../include/ternary_sa.h"
 #include "sa_common.h"
+#include "sa_jit.h"
 #include "sa_kernels.h"
 #include "sa_plan.h"
 
@@ -165,7 +166,68 @@ struct sa_handle {
   int64_t launches = 0;
   int32_t n_traced = 0;
   int64_t trace_steps = 0;
+  // statically scheduled kernel (sa_jit.h): device tables, the compiled kernel, the family choice
+  const uint32_t *d_lane_off2 = nullptr, *d_lane_meta = nullptr, *d_lane_clamp = nullptr, *d_wloc = nullptr, *d_thloc = nullptr;
+  const tsa::StaticKernel* sk = nullptr;
+  bool sk_tried = false;
+  int family = SA_KERNEL_AUTO;
+  std::string static_why;
 };
+
+namespace {
+
+int env_family(int family) {
+  if (const char* env = std::getenv("TSA_KERNEL")) {
+    const std::string e(env);
+    if (e == "generic" || e == "cta" || e == "warp") return SA_KERNEL_GENERIC;
+    if (e == "static") return SA_KERNEL_STATIC;
+  }
+  return family;
+}
+
+// Decide (once) whether sa_run uses the static kernel; compiles it on first use.
+bool use_static(sa_handle* h) {
+  const int fam = env_family(h->family);
+  if (fam == SA_KERNEL_GENERIC) return false;
+  if (!h->sk_tried) {
+    h->sk_tried = true;
+    h->sk = tsa::static_kernel_get(h->plan, tsa::StaticTuning::from_env(), &h->static_why);
+  }
+  return h->sk != nullptr;
+}
+
+tsa_static::Params static_params(const sa_handle* h, int64_t steps) {
+  tsa_static::Params q;
+  std::memset(&q, 0, sizeof(q));
+  q.lane_off2 = h->d_lane_off2; q.lane_meta = h->d_lane_meta; q.lane_clamp = h->d_lane_clamp;
+  q.initw = h->P.initw; q.obsw = h->P.obsw; q.obsm = h->P.obsm;
+  q.wloc = h->d_wloc; q.thloc = h->d_thloc;
+  std::memcpy(q.tha, h->P.tha, 16);
+  std::memcpy(q.thb, h->P.thb, 16);
+  q.fit_const = h->P.fit_const;
+  q.R = h->C.R;
+  q.cur_w = h->C.cur_w; q.cur_th = h->C.cur_th; q.best_w = h->C.best_w; q.best_th = h->C.best_th;
+  q.fit_cur = h->C.fit_cur; q.fit_best = h->C.fit_best;
+  q.key0 = h->S.key0; q.key1 = h->S.key1; q.chain_id_base = h->S.chain_id_base;
+  q.n_levels = h->S.n_levels; q.dmax = h->S.dmax; q.steps_per_level = h->S.steps_per_level;
+  q.accept = h->S.accept;
+  q.trace_row = h->Tr.row_of_chain; q.trace_rec = (tsa_static::u64*)h->Tr.records;
+  q.trace_max = h->Tr.max_steps; q.trace_g0 = h->Tr.g_start;
+  q.g0 = h->g; q.steps = steps;
+  return q;
+}
+
+tsa::PlanOptions plan_options(int64_t n_chains, int sm_count) {
+  tsa::PlanOptions o = tsa::PlanOptions::from_env();
+  if (!std::getenv("TSA_TEAM_MIN")) {
+    // few chains: spread each over more warps so that an SM still sees ~16 resident warps
+    const int64_t want = (16LL * sm_count + n_chains - 1) / std::max<int64_t>(n_chains, 1);
+    o.min_team_warps = (int)std::max<int64_t>(1, std::min<int64_t>(32, want));
+  }
+  return o;
+}
+
+}  // namespace
 
 extern "C" {
 
@@ -199,14 +261,22 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
   std::unique_ptr<sa_handle> h(new (std::nothrow) sa_handle());
   if (!h) return set_err(SA_ENOMEM, "host allocation failed");
   std::string err;
-  int rc = tsa::build_plan(net, obs, true, tsa::PlanOptions::from_env(), &h->plan, &err);
-  if (rc != SA_OK) return set_err(rc, err);
-
+  // argument errors are reported before device errors, so validation works without a GPU
   int dev = 0;
-  TSA_CUDA(cudaGetDevice(&dev));
-  TSA_CUDA(cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev));
+  cudaError_t dev_err = cudaGetDevice(&dev);
+  if (dev_err == cudaSuccess) dev_err = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
+  int rc = tsa::build_plan(net, obs, true, plan_options(sched->n_chains, h->sm_count), &h->plan, &err);
+  if (rc != SA_OK) return set_err(rc, err);
+  if (dev_err != cudaSuccess) return cuda_err(dev_err, "cudaGetDevice");
   cudaStream_t st = h->stream;
   if ((rc = upload_problem(h->plan, h->pool, &h->P, st))) return rc;
+  if (h->plan.team_warps > 0) {
+    if ((rc = h->pool.upload(h->plan.lane_off2, &h->d_lane_off2, st))) return rc;
+    if ((rc = h->pool.upload(h->plan.lane_meta, &h->d_lane_meta, st))) return rc;
+    if ((rc = h->pool.upload(h->plan.lane_clamp, &h->d_lane_clamp, st))) return rc;
+    if ((rc = h->pool.upload(h->plan.wloc, &h->d_wloc, st))) return rc;
+    if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
+  }
 
   const int R = sched->n_chains;
   tsa::DevChains& C = h->C;
@@ -258,6 +328,16 @@ int sa_run(sa_handle* h, int64_t steps) {
   if (!h) return set_err(SA_EINVAL, "null handle");
   if (steps < 0) return set_err(SA_EINVAL, "steps < 0");
   if (steps == 0) return SA_OK;
+  if (use_static(h)) {
+    const tsa_static::Params q = static_params(h, steps);
+    std::string why;
+    if (tsa::static_kernel_launch(h->sk, (unsigned)h->C.R, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
+    ++h->launches;
+    h->g += (uint64_t)steps;
+    return SA_OK;
+  }
+  if (env_family(h->family) == SA_KERNEL_STATIC)
+    return set_err(h->plan.team_warps > 0 ? SA_ECUDA : SA_EINVAL, "static kernel unavailable: " + h->static_why);
   if (h->warp_cpb > 0)
     TSA_CUDA(tsa::launch_run_warp(h->P, h->C, h->S, h->Tr, h->g, steps, h->warp_cpb, h->stream));
   else
@@ -415,6 +495,41 @@ int sa_get_trace(sa_handle* h, uint64_t* records) {
   return SA_OK;
 }
 
+int sa_select_kernel(sa_handle* h, int family) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  if (family != SA_KERNEL_AUTO && family != SA_KERNEL_GENERIC && family != SA_KERNEL_STATIC)
+    return set_err(SA_EINVAL, "unknown kernel family");
+  h->family = family;
+  return SA_OK;
+}
+
+int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_chains, int64_t info[8], char* log,
+                 size_t log_bytes) {
+  if (!net || !obs || !info || n_chains <= 0) return set_err(SA_EINVAL, "bad sa_jit_check arguments");
+  for (int i = 0; i < 8; ++i) info[i] = 0;
+  if (log && log_bytes) log[0] = 0;
+  auto put_log = [&](const std::string& s) {
+    if (log && log_bytes) { std::strncpy(log, s.c_str(), log_bytes - 1); log[log_bytes - 1] = 0; }
+  };
+  tsa::Plan pl;
+  std::string err;
+  const int rc = tsa::build_plan(net, obs, obs->obs != nullptr, plan_options(n_chains, 148), &pl, &err);
+  if (rc != SA_OK) return set_err(rc, err);
+  if (pl.team_warps <= 0) { put_log(pl.static_why); return SA_OK; }
+  info[0] = 1;
+  info[1] = pl.team_warps;
+  info[2] = pl.n_tiers;
+  for (int v : pl.tier_iters) info[3] += v;
+  info[5] = (int64_t)(((size_t)3 * pl.state_words * 4 + (size_t)pl.team_warps * 4 + 15) & ~(size_t)15);
+  std::string cubin, clog;
+  if (!tsa::static_kernel_compile(tsa::static_kernel_defines(pl, tsa::StaticTuning::from_env()), &cubin, &clog)) {
+    put_log(clog);
+    return set_err(SA_ECUDA, "static kernel did not compile: " + clog.substr(0, 400));
+  }
+  info[4] = (int64_t)cubin.size();
+  return SA_OK;
+}
+
 int sa_plan_info(const sa_network* net, const sa_observations* obs, int64_t info[16]) {
   if (!net || !obs || !info) return set_err(SA_EINVAL, "null argument");
   tsa::Plan pl;
@@ -444,6 +559,15 @@ int sa_get_info(sa_handle* h, int64_t info[16]) {
   info[2] = wk ? h->warp_cpb : 1;
   info[3] = wk ? (int64_t)tsa::warp_kernel_smem(h->P, h->warp_cpb) : (int64_t)tsa::smem_bytes(h->P);
   info[4] = wk ? (h->C.R + h->warp_cpb - 1) / h->warp_cpb : h->C.R;
+  if (h->sk && env_family(h->family) != SA_KERNEL_GENERIC) {
+    info[0] = 4;                                 // statically scheduled kernel: one team of W warps per chain
+    info[1] = h->sk->threads;
+    info[2] = 1;
+    info[3] = (int64_t)h->sk->smem_bytes;
+    info[4] = h->C.R;
+    info[14] = h->sk->regs;
+  }
+  info[15] = h->plan.team_warps;
   info[5] = h->P.Epad;
   info[6] = h->sm_count;
   info[7] = h->launches;

@@ -1,0 +1,43 @@
+// Run-time compilation of sa_static_kernel.cu for one problem's schedule (NVRTC, loaded with
+// dlopen) and its launch through the driver API (entry points from cudaGetDriverEntryPoint, so
+// libternary_sa.so links neither libnvrtc nor libcuda and still loads on a box without a GPU).
+#pragma once
+#include <cstddef>
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "sa_plan.h"
+#include "sa_static_params.h"
+
+namespace tsa {
+
+struct StaticTuning {
+  int max_regs = 128;     // register budget per thread -> __launch_bounds__ min blocks
+  int batch = 8;          // state gathers issued back to back before their IMADs
+  int t_unroll = 1;       // unroll factor of the time loop
+  static StaticTuning from_env();
+};
+
+// -D options of the kernel for this plan (the cache key of a compiled kernel).
+std::vector<std::string> static_kernel_defines(const Plan& plan, const StaticTuning& tune);
+
+// Compile only (no GPU needed).  Returns false with the NVRTC log / reason in *log.
+bool static_kernel_compile(const std::vector<std::string>& defines, std::string* cubin, std::string* log);
+
+struct StaticKernel {
+  void* module = nullptr;     // CUmodule
+  void* function = nullptr;   // CUfunction
+  int threads = 0;
+  size_t smem_bytes = 0;
+  int regs = 0;
+};
+
+// Compile (cached per process by the define list), load into the current context, and size the
+// dynamic shared memory.  Returns nullptr with the reason in *why.
+const StaticKernel* static_kernel_get(const Plan& plan, const StaticTuning& tune, std::string* why);
+
+// cuLaunchKernel on `stream`; returns a CUresult (0 = success) and the error text in *why.
+int static_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_static::Params& params, std::string* why);
+
+}  // namespace tsa

@@ -275,6 +275,9 @@ PlanOptions PlanOptions::from_env() {
   PlanOptions o;
   if (const char* e = std::getenv("TSA_NO_SPLIT")) o.split_rows = !(e[0] == '1');
   if (const char* e = std::getenv("TSA_NO_BANKOPT")) o.bank_opt = !(e[0] == '1');
+  if (const char* e = std::getenv("TSA_NO_TIERS")) o.tiers = !(e[0] == '1');
+  if (const char* e = std::getenv("TSA_TEAM_MIN")) o.min_team_warps = std::max(1, std::atoi(e));
+  if (const char* e = std::getenv("TSA_MAX_SLOTS")) o.max_lane_slots = std::max(0, std::atoi(e));
   return o;
 }
 
@@ -338,7 +341,10 @@ int build_plan(const sa_network* net, const sa_observations* obs, bool need_obs,
   p.n_chunks = (K + 4 * p.CG - 1) / (4 * p.CG);
   const int CG = p.CG, nb = p.nb;
   const int per_class = (N + nb - 1) / nb;
-  p.n_entries = nb * (1 + per_class);              // nb dummies first, then per_class entries per class
+  // nb zero dummies first, then per_class entries per class, then one scratch entry per lane (the
+  // static kernel lets lanes that finalise no node store there instead of predicating the store)
+  p.scratch_entry0 = nb * (1 + per_class);
+  p.n_entries = p.scratch_entry0 + 32;
   p.state_words = p.n_entries * CG;
   if ((size_t)p.state_words * 4 > 65535) return fail(err, "network too large for 16-bit state offsets (n_entries*CG*4 <= 65535)");
   for (int q = 0; q < NP; ++q) { p.tha[q] = (int8_t)(-net->th_lo[q]); p.thb[q] = (int8_t)(-net->th_hi[q] - 1); }
@@ -362,6 +368,52 @@ int build_plan(const sa_network* net, const sa_observations* obs, bool need_obs,
     std::vector<int> cls = assign_classes(lay, net->edge_src, N, CG, opt.bank_opt, &iters);
     const double cost = layout_cost(lay, iters);
     if (cost < best_cost) { best_cost = cost; best_lay = std::move(lay); best_cls = std::move(cls); best_iters = std::move(iters); }
+  }
+  // Tiers: order the passes by iteration count, give each of W warps one pass per tier, pad every
+  // pass to its tier's count.  One thread then holds sum(tier iterations) edge slots in registers.
+  int W = 0, NT = 0;
+  if (!opt.tiers) p.static_why = "tiers disabled";
+  else if (p.n_chunks != 1) p.static_why = "more than 16 conditions";
+  else {
+    for (int k = 0; k < K && p.static_why.empty(); ++k)
+      for (int i = 0; i < N; ++i)
+        if (obs->clamp[(size_t)k * N + i] && indeg[i] > 31) { p.static_why = "a clamped node has in-degree > 31"; break; }
+  }
+  if (p.static_why.empty()) {
+    const int np0 = (int)best_lay.passes.size();
+    std::vector<int> order(np0);
+    std::iota(order.begin(), order.end(), 0);
+    std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return best_iters[a] > best_iters[b]; });
+    const int max_slots = opt.max_lane_slots > 0 ? opt.max_lane_slots : (CG == 4 ? 40 : 48);
+    // W is a power of two (a 128-register budget then fills an SM's 512 threads with whole teams)
+    int w_lo = 1;
+    while (w_lo < std::min(opt.min_team_warps, 32) && 2 * w_lo <= np0) w_lo *= 2;
+    long best_cost = -1;
+    for (int w = w_lo; w <= 32 && (w == w_lo || w <= np0); w *= 2) {
+      const int nt = (np0 + w - 1) / w;
+      int slots = 0;
+      for (int j = 0; j < nt; ++j) slots += std::max(best_iters[order[j * w]], 1);
+      if (slots > max_slots) continue;
+      const long cost = (long)(slots + 4 * nt) * w;
+      if (best_cost < 0 || cost < best_cost) { best_cost = cost; W = w; NT = nt; }
+    }
+    if (W == 0) p.static_why = "too many edge slots per thread";
+    else {
+      Layout sorted;
+      std::vector<int> it2;
+      for (int x = 0; x < NT * W; ++x) {
+        if (x < np0) {
+          sorted.passes.push_back(std::move(best_lay.passes[order[x]]));
+          sorted.rounds.push_back(best_lay.rounds[order[x]]);
+        } else {
+          sorted.passes.push_back(std::vector<Row>(32));
+          sorted.rounds.push_back(0);
+        }
+        it2.push_back(std::max(best_iters[order[(x / W) * W]], 1));
+      }
+      best_lay = std::move(sorted);
+      best_iters = std::move(it2);
+    }
   }
   const Layout& lay = best_lay;
   p.n_pass = (int)lay.passes.size();
@@ -492,6 +544,65 @@ int build_plan(const sa_network* net, const sa_observations* obs, bool need_obs,
   if (p.fix.empty()) p.fix.push_back(0u);
   p.obs_idx_of_t.assign(T + 1, -1);
   for (int j = 0; j < NO; ++j) p.obs_idx_of_t[obs->obs_times[j]] = (int8_t)j;
+
+  // tables of the statically scheduled kernel: one column per thread (warp, lane) of the team
+  if (W > 0) {
+    p.team_warps = W;
+    p.n_tiers = NT;
+    const int TEAM = W * 32, EB = CG * 4;
+    for (int j = 0; j < NT; ++j) {
+      p.tier_iters.push_back(p.pass_iters[j * W]);
+      int r = 0;
+      for (int w = 0; w < W; ++w) r = std::max(r, lay.rounds[j * W + w]);
+      p.tier_rounds.push_back(r);
+    }
+    std::vector<int> wbase(NT + 1, 0);
+    for (int j = 0; j < NT; ++j) wbase[j + 1] = wbase[j] + (p.tier_iters[j] + 3) / 4;
+    auto slot_of = [&](int ps, int k, int lane) { return p.pass_base[ps] + (k / 4) * 128 + lane * 4 + (k % 4); };
+    for (int j = 0; j < NT; ++j) {
+      const int it = p.tier_iters[j];
+      for (int r = 0; r < (it + 1) / 2; ++r)
+        for (int th = 0; th < TEAM; ++th) {
+          const int ps = j * W + th / 32, lane = th % 32;
+          const uint32_t lo = p.slot_off[slot_of(ps, 2 * r, lane)];
+          const uint32_t hi = (2 * r + 1 < it) ? p.slot_off[slot_of(ps, 2 * r + 1, lane)] : 0u;
+          p.lane_off2.push_back(lo | (hi << 16));
+        }
+    }
+    p.lane_meta.assign((size_t)NT * TEAM, 0u);
+    p.lane_clamp.assign((size_t)NT * 3 * CG * TEAM, 0u);
+    p.thloc.assign(N, 0u);
+    for (int j = 0; j < NT; ++j)
+      for (int th = 0; th < TEAM; ++th) {
+        const int ps = j * W + th / 32, lane = th % 32;
+        const Row& r = lay.passes[ps][lane];
+        const uint32_t rm = p.row_meta[(size_t)ps * 32 + lane];
+        uint32_t meta = (uint32_t)((p.scratch_entry0 + lane) * EB);
+        if (r.node >= 0 && r.head) {
+          meta = (uint32_t)(p.entry_of_node[r.node] * EB) | kMetaHead;
+          p.thloc[r.node] = (uint32_t)j | ((uint32_t)th << 16);
+          for (int k = 0; k < K; ++k) {
+            if (!obs->clamp[(size_t)k * N + r.node]) continue;
+            const uint32_t v = obs->init_state[(size_t)k * N + r.node];
+            const int cg = k / 4, sh = 8 * (k % 4);
+            p.lane_clamp[((size_t)j * 3 * CG + cg) * TEAM + th] |= 0xFFu << sh;
+            p.lane_clamp[((size_t)j * 3 * CG + CG + cg) * TEAM + th] |= (v == 0 ? 64u : 192u) << sh;
+            p.lane_clamp[((size_t)j * 3 * CG + 2 * CG + cg) * TEAM + th] |= (v == 1 ? 128u : 0u) << sh;
+          }
+        }
+        meta |= rm & ~(kMetaOffMask | kMetaHead);          // the combine bits
+        p.lane_meta[(size_t)j * TEAM + th] = meta;
+      }
+    p.wloc.assign(E, 0u);
+    for (int e = 0; e < E; ++e) {
+      const int s = p.slot_of_param[e];
+      int ps = p.n_pass - 1;
+      while (p.pass_base[ps] > s) --ps;
+      const int rel = s - p.pass_base[ps], g = rel / 128, lane = (rel % 128) / 4, byte = rel % 4;
+      const int j = ps / W, th = (ps % W) * 32 + lane;
+      p.wloc[e] = (uint32_t)(wbase[j] + g) | ((uint32_t)byte << 8) | ((uint32_t)th << 16);
+    }
+  }
   return SA_OK;
 }
 

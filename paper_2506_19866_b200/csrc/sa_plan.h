@@ -14,6 +14,9 @@ namespace tsa {
 struct PlanOptions {
   bool split_rows = true;     // split long rows over consecutive lanes (TSA_NO_SPLIT=1 disables)
   bool bank_opt = true;       // optimise bank classes by hill climbing (TSA_NO_BANKOPT=1 disables)
+  bool tiers = true;          // group the passes into tiers for the statically scheduled kernel (TSA_NO_TIERS=1 disables)
+  int min_team_warps = 1;     // lower bound of warps per chain (few chains: spread each over more warps)
+  int max_lane_slots = 0;     // edge slots one thread may hold in registers; 0 = default for the CG
   static PlanOptions from_env();
 };
 
@@ -37,6 +40,18 @@ struct Plan {
   int8_t tha[16] = {0}, thb[16] = {0};
   // statistics for sa_get_info / DESIGN.md
   int total_iters = 0, n_rows = 0, n_split_nodes = 0;
+
+  // Static schedule (sa_static_kernel.cu).  team_warps = W > 0: the passes are ordered tier-major
+  // (pass = tier*W + warp), all passes of a tier have the tier's iteration count, and the tables
+  // below hold one column per thread of the team.  W = 0: not applicable, static_why says why.
+  int team_warps = 0, n_tiers = 0, scratch_entry0 = 0;
+  std::string static_why;
+  std::vector<int32_t> tier_iters, tier_rounds;           // [n_tiers]
+  std::vector<uint32_t> lane_off2;                        // [sum ceil(it/2)][W*32]
+  std::vector<uint32_t> lane_meta;                        // [n_tiers][W*32]
+  std::vector<uint32_t> lane_clamp;                       // [n_tiers][3*CG][W*32]: mask, A bytes, D bytes of clamped lanes
+  std::vector<uint32_t> wloc;                             // [E]
+  std::vector<uint32_t> thloc;                            // [N]
 
   // caller order (int8 [E+N]) <-> internal rows (w [EpadA], th [NpadA])
   void to_internal(const int8_t* params, int8_t* w, int8_t* th) const;
