@@ -119,7 +119,7 @@ int sa_geometric_table(double t0, double t_end, int32_t n_levels, int32_t dmax, 
 
 /* Which kernel family a handle uses and how it was launched (for bench.py / DESIGN.md):
  * info[0] = sa_run kernel variant (2 = generic, CTA per chain; 3 = generic, warp per chain;
- * 4 = statically scheduled), [1] = threads per CTA, [2] = chains per CTA, [3] = dynamic shared
+ * 4 = statically scheduled, 5 = dense / tensor pipe), [1] = threads per CTA, [2] = chains per CTA, [3] = dynamic shared
  * memory bytes per CTA, [4] = CTAs in the sa_run grid, [5] = edge slots per chain (padded),
  * [6] = SM count, [7] = kernels launched so far by this handle, [8] = passes per time step,
  * [9] = edge iterations per time step (sum over passes), [10] = rows, [11] = split nodes,
@@ -128,21 +128,24 @@ int sa_geometric_table(double t0, double t_end, int32_t n_levels, int32_t dmax, 
  * The variant is decided at the first sa_run; before it, info[0] reports the generic choice. */
 int sa_get_info(sa_handle *h, int64_t info[16]);
 
-/* Kernel family of sa_run.  AUTO (default): the statically scheduled kernel — edge schedule,
- * weights and thresholds in registers, compiled for this problem's schedule by NVRTC at the first
- * sa_run — when it applies and NVRTC is available, else the generic one.  GENERIC:
- * the ahead-of-time compiled table-driven kernels.  STATIC: like AUTO but sa_run fails with
- * SA_EINVAL / SA_ECUDA (reason in sa_last_error) instead of falling back.  Both families produce
- * identical results.  Environment override: TSA_KERNEL=generic|static. */
+/* Kernel family of sa_run.  AUTO (default): the dense kernel — the node update as an int8 product
+ * on the tensor pipe with the chain's weight matrix in mma.sync fragments — when the
+ * network has at most 128 nodes and 8 conditions; else the statically scheduled gather kernel —
+ * edge schedule, weights and thresholds in registers — when it applies; both are compiled for the
+ * problem at hand by NVRTC at the first sa_run.  Else the generic one.  GENERIC: the ahead-of-time
+ * compiled table-driven kernels.  STATIC / DENSE: that family only; sa_run fails with SA_EINVAL /
+ * SA_ECUDA (reason in sa_last_error) instead of falling back.  All families produce identical
+ * results.  Environment override: TSA_KERNEL=generic|static|dense. */
 #define SA_KERNEL_AUTO    0
 #define SA_KERNEL_GENERIC 1
 #define SA_KERNEL_STATIC  2
+#define SA_KERNEL_DENSE   3
 int sa_select_kernel(sa_handle *h, int family);
 
 /* Host only (no GPU needed): build the plan of a problem for n_chains chains and compile the
  * statically scheduled kernel for it.  info[0] = 1 if the static kernel applies, [1] = warps per
  * chain, [2] = tiers, [3] = edge slots per thread, [4] = cubin bytes, [5] = shared memory bytes per
- * CTA; log (may be NULL) receives the reason / NVRTC log, truncated to log_bytes.  Returns SA_OK
+ * CTA, [6] = 1 if the dense kernel applies, [7] = its cubin bytes; log (may be NULL) receives the reason / NVRTC log, truncated to log_bytes.  Returns SA_OK
  * also when the kernel does not apply (info[0] = 0); SA_ECUDA when NVRTC is missing or fails. */
 int sa_jit_check(const sa_network *net, const sa_observations *obs, int32_t n_chains, int64_t info[8],
                  char *log, size_t log_bytes);

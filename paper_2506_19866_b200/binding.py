@@ -21,7 +21,7 @@ EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simula
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info",
            "sa_select_kernel", "sa_jit_check")
-SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC = 0, 1, 2
+SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2506_19866_b200.build` "
@@ -250,7 +250,8 @@ def sa_jit_check(prob, n_chains: int) -> dict:
     log = C.create_string_buffer(16384)
     _check(_lib.sa_jit_check(C.byref(net), C.byref(obs), n_chains, info.ctypes.data, log, len(log)), "sa_jit_check")
     return {"applies": bool(info[0]), "team_warps": int(info[1]), "tiers": int(info[2]), "lane_slots": int(info[3]),
-            "cubin_bytes": int(info[4]), "smem_bytes": int(info[5]), "log": log.value.decode(errors="replace")}
+            "cubin_bytes": int(info[4]), "smem_bytes": int(info[5]), "dense_applies": bool(info[6]),
+            "dense_cubin_bytes": int(info[7]), "log": log.value.decode(errors="replace")}
 
 
 def sa_int32_peak() -> dict:

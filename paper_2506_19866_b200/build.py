@@ -11,8 +11,10 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libternary_sa.so")
-SOURCES = ["sa_api.cu", "sa_kernels.cu", "sa_peak.cu", "sa_plan.cpp", "sa_jit.cpp", "sa_static_aot.cu"]
-EMBED = os.path.join(CSRC, "sa_static_source.inc")
+SOURCES = ["sa_api.cu", "sa_kernels.cu", "sa_peak.cu", "sa_plan.cpp", "sa_dense_plan.cpp", "sa_jit.cpp", "sa_static_aot.cu",
+           "sa_dense_aot.cu"]
+EMBED = {"sa_static_source.inc": ("sa_static_params.h", "sa_static_kernel.cu"),
+         "sa_dense_source.inc": ("sa_dense_params.h", "sa_dense_kernel.cu")}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "--use_fast_math"]
 
@@ -39,18 +41,20 @@ def stale() -> bool:
 def embed_static_source() -> None:
     """sa_static_source.inc = params header + kernel source as one C++ raw string literal: the
     text NVRTC compiles at run time (sa_jit.cpp)."""
-    parts = []
-    for name in ("sa_static_params.h", "sa_static_kernel.cu"):
-        with open(os.path.join(CSRC, name)) as f:
-            parts.append(f.read())
-    text = 'R"TSASRC(' + "\n".join(parts) + ')TSASRC"\n'
-    old = None
-    if os.path.exists(EMBED):
-        with open(EMBED) as f:
-            old = f.read()
-    if old != text:
-        with open(EMBED, "w") as f:
-            f.write(text)
+    for inc, names in EMBED.items():
+        parts = []
+        for name in names:
+            with open(os.path.join(CSRC, name)) as f:
+                parts.append(f.read())
+        text = 'R"TSASRC(' + "\n".join(parts) + ')TSASRC"\n'
+        path = os.path.join(CSRC, inc)
+        old = None
+        if os.path.exists(path):
+            with open(path) as f:
+                old = f.read()
+        if old != text:
+            with open(path, "w") as f:
+                f.write(text)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

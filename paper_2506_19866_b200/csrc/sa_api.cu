@@ -170,6 +170,13 @@ struct sa_handle {
   const uint32_t *d_lane_off2 = nullptr, *d_lane_meta = nullptr, *d_lane_clamp = nullptr, *d_wloc = nullptr, *d_thloc = nullptr;
   const tsa::StaticKernel* sk = nullptr;
   bool sk_tried = false;
+  // dense (tensor-pipe) kernel (sa_dense_plan.h): host tables, device tables, the compiled kernel
+  tsa::DensePlan dplan;
+  const uint16_t *d_frag_slot = nullptr, *d_th_entry = nullptr;
+  const uint32_t *d_init_frag = nullptr, *d_obs_word = nullptr, *d_fix = nullptr, *d_dwloc = nullptr, *d_dthloc = nullptr;
+  const tsa::StaticKernel* dk = nullptr;
+  bool dk_tried = false;
+  std::string dense_why;
   int family = SA_KERNEL_AUTO;
   std::string static_why;
 };
@@ -181,14 +188,46 @@ int env_family(int family) {
     const std::string e(env);
     if (e == "generic" || e == "cta" || e == "warp") return SA_KERNEL_GENERIC;
     if (e == "static") return SA_KERNEL_STATIC;
+    if (e == "dense") return SA_KERNEL_DENSE;
   }
   return family;
+}
+
+// Decide (once) whether sa_run uses the dense kernel; compiles it on first use.
+bool use_dense(sa_handle* h) {
+  const int fam = env_family(h->family);
+  if (fam != SA_KERNEL_AUTO && fam != SA_KERNEL_DENSE) return false;
+  if (!h->dk_tried) {
+    h->dk_tried = true;
+    h->dk = tsa::dense_kernel_get(h->plan, h->dplan, tsa::StaticTuning::from_env(), &h->dense_why);
+  }
+  return h->dk != nullptr;
+}
+
+tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
+  tsa_dense::Params q;
+  std::memset(&q, 0, sizeof(q));
+  q.frag_slot = h->d_frag_slot; q.th_entry = h->d_th_entry; q.init_frag = h->d_init_frag;
+  q.obs_word = h->d_obs_word; q.fix = h->d_fix; q.wloc = h->d_dwloc; q.thloc = h->d_dthloc;
+  std::memcpy(q.tha, h->P.tha, 16);
+  std::memcpy(q.thb, h->P.thb, 16);
+  q.fit_const = h->dplan.fit_const;
+  q.R = h->C.R;
+  q.cur_w = h->C.cur_w; q.cur_th = h->C.cur_th; q.best_w = h->C.best_w; q.best_th = h->C.best_th;
+  q.fit_cur = h->C.fit_cur; q.fit_best = h->C.fit_best;
+  q.key0 = h->S.key0; q.key1 = h->S.key1; q.chain_id_base = h->S.chain_id_base;
+  q.n_levels = h->S.n_levels; q.dmax = h->S.dmax; q.steps_per_level = h->S.steps_per_level;
+  q.accept = h->S.accept;
+  q.trace_row = h->Tr.row_of_chain; q.trace_rec = (tsa_dense::u64*)h->Tr.records;
+  q.trace_max = h->Tr.max_steps; q.trace_g0 = h->Tr.g_start;
+  q.g0 = h->g; q.steps = steps;
+  return q;
 }
 
 // Decide (once) whether sa_run uses the static kernel; compiles it on first use.
 bool use_static(sa_handle* h) {
   const int fam = env_family(h->family);
-  if (fam == SA_KERNEL_GENERIC) return false;
+  if (fam == SA_KERNEL_GENERIC || fam == SA_KERNEL_DENSE) return false;
   if (!h->sk_tried) {
     h->sk_tried = true;
     h->sk = tsa::static_kernel_get(h->plan, tsa::StaticTuning::from_env(), &h->static_why);
@@ -277,6 +316,16 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->plan.wloc, &h->d_wloc, st))) return rc;
     if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
   }
+  tsa::build_dense_plan(net, obs, h->plan, &h->dplan);
+  if (h->dplan.ok) {
+    if ((rc = h->pool.upload(h->dplan.frag_slot, &h->d_frag_slot, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.th_entry, &h->d_th_entry, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.init_frag, &h->d_init_frag, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.obs_word, &h->d_obs_word, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.fix, &h->d_fix, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.wloc, &h->d_dwloc, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.thloc, &h->d_dthloc, st))) return rc;
+  }
 
   const int R = sched->n_chains;
   tsa::DevChains& C = h->C;
@@ -328,6 +377,16 @@ int sa_run(sa_handle* h, int64_t steps) {
   if (!h) return set_err(SA_EINVAL, "null handle");
   if (steps < 0) return set_err(SA_EINVAL, "steps < 0");
   if (steps == 0) return SA_OK;
+  if (use_dense(h)) {
+    const tsa_dense::Params q = dense_params(h, steps);
+    std::string why;
+    if (tsa::dense_kernel_launch(h->dk, (unsigned)h->C.R, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
+    ++h->launches;
+    h->g += (uint64_t)steps;
+    return SA_OK;
+  }
+  if (env_family(h->family) == SA_KERNEL_DENSE)
+    return set_err(h->dplan.ok ? SA_ECUDA : SA_EINVAL, "dense kernel unavailable: " + h->dense_why);
   if (use_static(h)) {
     const tsa_static::Params q = static_params(h, steps);
     std::string why;
@@ -497,7 +556,7 @@ int sa_get_trace(sa_handle* h, uint64_t* records) {
 
 int sa_select_kernel(sa_handle* h, int family) {
   if (!h) return set_err(SA_EINVAL, "null handle");
-  if (family != SA_KERNEL_AUTO && family != SA_KERNEL_GENERIC && family != SA_KERNEL_STATIC)
+  if (family != SA_KERNEL_AUTO && family != SA_KERNEL_GENERIC && family != SA_KERNEL_STATIC && family != SA_KERNEL_DENSE)
     return set_err(SA_EINVAL, "unknown kernel family");
   h->family = family;
   return SA_OK;
@@ -515,6 +574,19 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
   std::string err;
   const int rc = tsa::build_plan(net, obs, obs->obs != nullptr, plan_options(n_chains, 148), &pl, &err);
   if (rc != SA_OK) return set_err(rc, err);
+  {
+    tsa::DensePlan dp;
+    tsa::build_dense_plan(net, obs, pl, &dp);
+    if (dp.ok) {
+      info[6] = 1;
+      std::string cubin, clog;
+      if (!tsa::dense_kernel_compile(tsa::dense_kernel_defines(pl, dp, tsa::StaticTuning::from_env()), &cubin, &clog)) {
+        put_log(clog);
+        return set_err(SA_ECUDA, "dense kernel did not compile: " + clog.substr(0, 400));
+      }
+      info[7] = (int64_t)cubin.size();
+    }
+  }
   if (pl.team_warps <= 0) { put_log(pl.static_why); return SA_OK; }
   info[0] = 1;
   info[1] = pl.team_warps;
@@ -568,6 +640,15 @@ int sa_get_info(sa_handle* h, int64_t info[16]) {
     info[14] = h->sk->regs;
   }
   info[15] = h->plan.team_warps;
+  if (h->dk && (env_family(h->family) == SA_KERNEL_AUTO || env_family(h->family) == SA_KERNEL_DENSE)) {
+    info[0] = 5;                                 // dense kernel: one warp per chain, W in mma.sync A fragments
+    info[1] = h->dk->threads;
+    info[2] = 1;
+    info[3] = (int64_t)h->dk->smem_bytes;
+    info[4] = h->C.R;
+    info[14] = h->dk->regs;
+    info[15] = 1;
+  }
   info[5] = h->P.Epad;
   info[6] = h->sm_count;
   info[7] = h->launches;

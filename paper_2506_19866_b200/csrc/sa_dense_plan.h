@@ -1,0 +1,35 @@
+// Host-side tables of the dense (tensor-pipe) sa_run kernel, sa_dense_kernel.cu: where every
+// candidate edge sits in the mma.sync A fragments, the row <-> column numbering that makes the
+// C -> B fragment exchange two vector stores and two vector loads, the observation words in the
+// layout of a lane's result words, clamp fix-ups.  Pure host C++; deterministic.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+#include "sa_plan.h"
+
+namespace tsa {
+
+struct DensePlan {
+  bool ok = false;
+  std::string why;          // reason when !ok
+  int MT = 0, KS = 0;       // 16-row tiles, 32-column steps (KS = words per condition a lane produces)
+  int CS = 0, TS = 0;       // byte strides of the exchange buffer: per condition, per B-fragment thread chunk
+  int exchange_wavefronts = 0;   // shared-memory wavefronts of one exchange (2 stores + 2 loads)
+  int n_fix_rounds = 1;
+  int fit_const = 0;
+  std::vector<uint16_t> frag_slot;   // [MT*KS*4][32][4]
+  std::vector<uint16_t> th_entry;    // [8][KS][4]
+  std::vector<uint32_t> init_frag;   // [32][2*KS]
+  std::vector<uint32_t> obs_word;    // [n_obs][32][2*KS]
+  std::vector<uint32_t> fix;         // [n_fix_rounds][32]
+  std::vector<uint32_t> wloc;        // [E]
+  std::vector<uint32_t> thloc;       // [N]
+  size_t smem_bytes(const Plan& pl) const { return (size_t)8 * CS + (size_t)pl.EpadA + (size_t)pl.NpadA; }
+};
+
+// Applies when N <= 128 and K <= 8.  Always returns; check dp->ok / dp->why.
+void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& plan, DensePlan* dp);
+
+}  // namespace tsa

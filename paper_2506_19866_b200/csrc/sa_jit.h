@@ -7,6 +7,8 @@
 #include <string>
 #include <vector>
 
+#include "sa_dense_params.h"
+#include "sa_dense_plan.h"
 #include "sa_plan.h"
 #include "sa_static_params.h"
 
@@ -16,6 +18,7 @@ struct StaticTuning {
   int max_regs = 128;     // register budget per thread -> __launch_bounds__ min blocks
   int batch = 8;          // state gathers issued back to back before their IMADs
   int t_unroll = 1;       // unroll factor of the time loop
+  int dense_blocks = 10;  // dense kernel: resident one-warp CTAs per SM the register allocation aims at
   static StaticTuning from_env();
 };
 
@@ -39,5 +42,11 @@ const StaticKernel* static_kernel_get(const Plan& plan, const StaticTuning& tune
 
 // cuLaunchKernel on `stream`; returns a CUresult (0 = success) and the error text in *why.
 int static_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_static::Params& params, std::string* why);
+
+// The dense (tensor-pipe) kernel, sa_dense_kernel.cu: same cache, loader and launch path.
+std::vector<std::string> dense_kernel_defines(const Plan& plan, const DensePlan& dp, const StaticTuning& tune);
+bool dense_kernel_compile(const std::vector<std::string>& defines, std::string* cubin, std::string* log);
+const StaticKernel* dense_kernel_get(const Plan& plan, const DensePlan& dp, const StaticTuning& tune, std::string* why);
+int dense_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_dense::Params& params, std::string* why);
 
 }  // namespace tsa
