@@ -316,7 +316,7 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->plan.wloc, &h->d_wloc, st))) return rc;
     if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
   }
-  tsa::build_dense_plan(net, obs, h->plan, &h->dplan);
+  tsa::build_dense_plan(net, obs, h->plan, tsa::StaticTuning::from_env().dense_warps, &h->dplan);
   if (h->dplan.ok) {
     if ((rc = h->pool.upload(h->dplan.frag_slot, &h->d_frag_slot, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.th_entry, &h->d_th_entry, st))) return rc;
@@ -576,7 +576,7 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
   if (rc != SA_OK) return set_err(rc, err);
   {
     tsa::DensePlan dp;
-    tsa::build_dense_plan(net, obs, pl, &dp);
+    tsa::build_dense_plan(net, obs, pl, tsa::StaticTuning::from_env().dense_warps, &dp);
     if (dp.ok) {
       info[6] = 1;
       std::string cubin, clog;
@@ -647,7 +647,7 @@ int sa_get_info(sa_handle* h, int64_t info[16]) {
     info[3] = (int64_t)h->dk->smem_bytes;
     info[4] = h->C.R;
     info[14] = h->dk->regs;
-    info[15] = 1;
+    info[15] = h->dplan.W;
   }
   info[5] = h->P.Epad;
   info[6] = h->sm_count;

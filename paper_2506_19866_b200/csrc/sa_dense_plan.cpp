@@ -30,21 +30,23 @@ int wavefronts(const int (&addr)[32], int vec_bytes) {
 
 // Strides (CS per condition, TS per B-thread chunk) of the exchange buffer with the fewest
 // wavefronts for the kernel's two stores and two loads.
-void pick_strides(int KS, int* CS, int* TS, int* wf) {
-  const int NW = KS, vec = NW * 4;
+void pick_strides(int KS, int W, int* CS, int* TS, int* wf) {
+  const int NW = KS, vec = NW * 4, WPW = NW / W, svec = WPW * 4;
   int best = 1 << 30;
   for (int ts = 2 * KS * 4; ts <= 2 * KS * 4 + 128; ts += 4) {
     if (ts % vec) continue;
     for (int cs = 4 * ts; cs <= 4 * ts + 256; cs += 4) {
       if (cs % vec || (8 * cs) % 16) continue;
       int w = 0, addr[32];
-      for (int c = 0; c < 2; ++c) {
-        for (int l = 0; l < 32; ++l) addr[l] = (2 * (l % 4) + c) * cs + ((l / 4) % 4) * ts + ((l / 4) / 4) * NW * 4;
-        w += wavefronts(addr, vec);
-      }
+      for (int c = 0; c < 2; ++c)
+        for (int ww = 0; ww < W; ++ww) {
+          for (int l = 0; l < 32; ++l)
+            addr[l] = (2 * (l % 4) + c) * cs + ((l / 4) % 4) * ts + (((l / 4) / 4) * NW + ww * WPW) * 4;
+          w += wavefronts(addr, svec);
+        }
       for (int half = 0; half < 2; ++half) {
         for (int l = 0; l < 32; ++l) addr[l] = (l / 4) * cs + (l % 4) * ts + half * NW * 4;
-        w += wavefronts(addr, vec);
+        w += W * wavefronts(addr, vec);
       }
       if (w < best) { best = w; *CS = cs; *TS = ts; }
     }
@@ -54,7 +56,7 @@ void pick_strides(int KS, int* CS, int* TS, int* wf) {
 
 }  // namespace
 
-void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& pl, DensePlan* dp) {
+void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& pl, int team_warps, DensePlan* dp) {
   *dp = DensePlan();
   const int N = pl.N, E = pl.E, K = pl.K, NO = pl.n_obs;
   if (N > 128) { dp->why = "more than 128 nodes"; return; }
@@ -64,8 +66,11 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   int KS = (MT + 1) / 2;
   if (KS == 3) KS = 4;
   const int NW = KS;
-  dp->MT = MT; dp->KS = KS;
-  pick_strides(KS, &dp->CS, &dp->TS, &dp->exchange_wavefronts);
+  int W = team_warps >= 4 ? 4 : team_warps >= 2 ? 2 : 1;
+  while (W > KS) W /= 2;
+  const int WPW = NW / W, MTW = 2 * WPW;
+  dp->MT = MT; dp->KS = KS; dp->W = W;
+  pick_strides(KS, W, &dp->CS, &dp->TS, &dp->exchange_wavefronts);
   const int CS = dp->CS, TS = dp->TS;
 
   // Row r = 16m + 8h + g is produced by thread group g as byte j of its word w, q = 2m + h = 4w + j.
@@ -83,13 +88,14 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   std::vector<int> node_of_col(32 * KS, -1);
   for (int i = 0; i < N; ++i) node_of_col[col_of_row(i)] = i;
 
-  // A fragments: register (m, s, a) of lane (g, t) holds row 16m + g + 8(a&1), columns 32s + 16(a>>1) + 4t + 0..3
+  // A fragments: register (m, s, a) of lane (g, t) holds row 16m + g + 8(a&1), columns 32s + 16(a>>1) + 4t + 0..3;
+  // row tile m belongs to warp m / MTW as its tile m % MTW
   std::map<std::pair<int, int>, int> edge_at;       // (dst, src) -> edge
   for (int e = 0; e < E; ++e) edge_at[{net->edge_dst[e], net->edge_src[e]}] = e;
-  const int NA = MT * KS * 4;
+  const int NA = 2 * NW * KS * 4;
   dp->frag_slot.assign((size_t)NA * 32 * 4, 0xFFFFu);
   dp->wloc.assign(E, 0u);
-  for (int m = 0; m < MT; ++m)
+  for (int m = 0; m < 2 * NW; ++m)
     for (int s = 0; s < KS; ++s)
       for (int a = 0; a < 4; ++a)
         for (int lane = 0; lane < 32; ++lane)
@@ -101,7 +107,8 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
             if (it == edge_at.end()) continue;
             const int e = it->second, slot = pl.slot_of_param[e];
             dp->frag_slot[((size_t)reg * 32 + lane) * 4 + b] = (uint16_t)slot;
-            dp->wloc[e] = (uint32_t)reg | ((uint32_t)b << 8) | ((uint32_t)lane << 10) | ((uint32_t)slot << 16);
+            const int ww = m / MTW, wreg = ((m % MTW) * KS + s) * 4 + a;
+            dp->wloc[e] = (uint32_t)wreg | ((uint32_t)b << 7) | ((uint32_t)lane << 9) | ((uint32_t)ww << 14) | ((uint32_t)slot << 16);
           }
   // thresholds: byte j of word w of thread group g <-> row
   dp->th_entry.assign((size_t)8 * NW * 4, 0xFFFFu);
@@ -125,14 +132,18 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
         dp->init_frag[(size_t)lane * 2 * KS + x] |= (uint32_t)obs->init_state[(size_t)cond * N + node_of_col[col]] << (8 * j);
       }
   // clamped (condition, node): restored by a byte store after every exchange; scored once, here
-  std::vector<uint32_t> fixes;
+  // (the warp that owns the row's result word stores it, right after its own vector stores)
+  std::vector<std::vector<uint32_t>> fixes(W);
   for (int k = 0; k < K; ++k)
     for (int i = 0; i < N; ++i)
-      if (obs->clamp[(size_t)k * N + i])
-        fixes.push_back((uint32_t)state_offset(k, i) | ((uint32_t)obs->init_state[(size_t)k * N + i] << 16) | 0x80000000u);
-  dp->n_fix_rounds = std::max(1, (int)(fixes.size() + 31) / 32);
-  dp->fix.assign((size_t)dp->n_fix_rounds * 32, 0u);
-  std::copy(fixes.begin(), fixes.end(), dp->fix.begin());
+      if (obs->clamp[(size_t)k * N + i]) {
+        const int q = 2 * (i / 16) + (i % 16) / 8, ww = (q / 4) / WPW;
+        fixes[ww].push_back((uint32_t)state_offset(k, i) | ((uint32_t)obs->init_state[(size_t)k * N + i] << 16) | 0x80000000u);
+      }
+  dp->n_fix_rounds = 1;
+  for (int ww = 0; ww < W; ++ww) dp->n_fix_rounds = std::max(dp->n_fix_rounds, (int)(fixes[ww].size() + 31) / 32);
+  dp->fix.assign((size_t)W * dp->n_fix_rounds * 32, 0u);
+  for (int ww = 0; ww < W; ++ww) std::copy(fixes[ww].begin(), fixes[ww].end(), dp->fix.begin() + (size_t)ww * dp->n_fix_rounds * 32);
   // observations in the layout of a lane's result words; 3 = never equal to a state, so such an
   // entry always counts one mismatch, which fit_const takes back
   dp->obs_word.assign((size_t)NO * 32 * 2 * NW, 0x03030303u);

@@ -14,22 +14,26 @@ namespace tsa {
 struct DensePlan {
   bool ok = false;
   std::string why;          // reason when !ok
-  int MT = 0, KS = 0;       // 16-row tiles, 32-column steps (KS = words per condition a lane produces)
+  int MT = 0, KS = 0;       // 16-row tiles, 32-column steps (KS = result words per condition and thread group)
+  int W = 1;                // warps per chain; warp ww owns result words ww*KS/W .. and their row tiles
   int CS = 0, TS = 0;       // byte strides of the exchange buffer: per condition, per B-fragment thread chunk
   int exchange_wavefronts = 0;   // shared-memory wavefronts of one exchange (2 stores + 2 loads)
   int n_fix_rounds = 1;
   int fit_const = 0;
-  std::vector<uint16_t> frag_slot;   // [MT*KS*4][32][4]
+  std::vector<uint16_t> frag_slot;   // [2*KS*KS*4][32][4] (row tiles padded to 2*KS)
   std::vector<uint16_t> th_entry;    // [8][KS][4]
   std::vector<uint32_t> init_frag;   // [32][2*KS]
   std::vector<uint32_t> obs_word;    // [n_obs][32][2*KS]
-  std::vector<uint32_t> fix;         // [n_fix_rounds][32]
+  std::vector<uint32_t> fix;         // [W][n_fix_rounds][32]
   std::vector<uint32_t> wloc;        // [E]
   std::vector<uint32_t> thloc;       // [N]
-  size_t smem_bytes(const Plan& pl) const { return (size_t)8 * CS + (size_t)pl.EpadA + (size_t)pl.NpadA; }
+  size_t smem_bytes(const Plan& pl) const {
+    return (size_t)(W > 1 ? 2 : 1) * 8 * CS + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)2 * W * 4;
+  }
 };
 
-// Applies when N <= 128 and K <= 8.  Always returns; check dp->ok / dp->why.
-void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& plan, DensePlan* dp);
+// Applies when N <= 128 and K <= 8.  team_warps = warps per chain (1, 2 or 4; reduced until it
+// divides KS).  Always returns; check dp->ok / dp->why.
+void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& plan, int team_warps, DensePlan* dp);
 
 }  // namespace tsa

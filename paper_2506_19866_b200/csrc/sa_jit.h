@@ -18,7 +18,8 @@ struct StaticTuning {
   int max_regs = 128;     // register budget per thread -> __launch_bounds__ min blocks
   int batch = 8;          // state gathers issued back to back before their IMADs
   int t_unroll = 1;       // unroll factor of the time loop
-  int dense_blocks = 10;  // dense kernel: resident one-warp CTAs per SM the register allocation aims at
+  int dense_blocks = 8;   // dense kernel: resident chains (CTAs) per SM the register allocation aims at
+  int dense_warps = 1;    // dense kernel: warps per chain (1, 2 or 4); 1 measured fastest at every R
   static StaticTuning from_env();
 };
 
