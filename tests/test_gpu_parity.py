@@ -227,6 +227,7 @@ def test_split_runs_chain_base_and_team_width(B, problems_cache):
         os.environ.update(env)
         try:
             with Handle(B, prob, sched) as d:
+                B.sa_select_kernel(d.h, B.SA_KERNEL_GENERIC if "TSA_TEAM_WARPS" in env else B.SA_KERNEL_STATIC)
                 info = B.sa_get_info(d.h)
                 if "TSA_TEAM_WARPS" in env:
                     assert info["threads_per_cta"] == 32 * int(env["TSA_TEAM_WARPS"])
@@ -240,6 +241,62 @@ def test_split_runs_chain_base_and_team_width(B, problems_cache):
         finally:
             for k in env:
                 del os.environ[k]
+
+
+FAMILY_CASES = [
+    # problem, family, environment
+    ("hpg", "GENERIC", {}), ("hpg", "STATIC", {}), ("hpg", "DENSE", {}),
+    ("mtb", "GENERIC", {}), ("mtb", "STATIC", {}), ("mtb", "DENSE", {}),
+    ("mtb", "DENSE", {"TSA_DENSE_W": "2"}), ("mtb", "DENSE", {"TSA_DENSE_W": "4"}),
+    ("mtb", "DENSE", {"TSA_DENSE_BLOCKS": "12"}),
+]
+
+
+@pytest.mark.parametrize("name,family,env", FAMILY_CASES, ids=[f"{n}-{f}-{'-'.join(e.values()) or 'default'}" for n, f, e in FAMILY_CASES])
+def test_every_kernel_family_matches_the_oracle(B, problems_cache, name, family, env):
+    """sa_run has three kernel families (include/ternary_sa.h); each one, forced, reproduces the
+    oracle's trace, vectors and fitness, and says which one ran."""
+    prob = problems_cache(name)
+    orc = O.Oracle(prob)
+    sched = PB.default_schedule(name, n_chains=24, total_steps=400)
+    chains = [0, 1, 7, 23]
+    os.environ.update(env)
+    try:
+        with Handle(B, prob, sched) as hd:
+            B.sa_select_kernel(hd.h, getattr(B, "SA_KERNEL_" + family))
+            B.sa_set_trace(hd.h, chains, 400)
+            B.sa_run(hd.h, 130)
+            B.sa_run(hd.h, 270)
+            info = B.sa_get_info(hd.h)
+            assert info["variant"] == {"GENERIC": info["variant"], "STATIC": 4, "DENSE": 5}[family]
+            assert family != "GENERIC" or info["variant"] in (2, 3)
+            if "TSA_DENSE_W" in env:
+                assert info["threads_per_cta"] == 32 * int(env["TSA_DENSE_W"])
+            check_chains(B, hd, orc, chains, 400, B.sa_get_trace(hd.h, len(chains), 400))
+            check_all_fitness(B, hd, orc)
+    finally:
+        for k in env:
+            del os.environ[k]
+
+
+def test_dense_kernel_limits(B):
+    """The dense family applies up to 128 nodes and 8 conditions; beyond that DENSE fails loudly
+    and AUTO falls back to the gather kernels with identical results."""
+    for name, N, E, K in (("n128", 128, 700, 8), ("n129", 129, 700, 8), ("k9", 40, 160, 9)):
+        cs = PB.ConfigSpec(name, 777 + N + K, N, E, "poisson", K, 2, 10, (5, 10), 8, 200, max_in_degree=40)
+        prob = PB.make_problem(name, O.simulate_fn, spec=cs, noise=0.05)
+        orc = O.Oracle(prob)
+        sched = PB.make_schedule(8, 200)
+        with Handle(B, prob, sched) as hd:
+            B.sa_set_trace(hd.h, list(range(8)), 200)
+            B.sa_run(hd.h, 200)
+            assert (B.sa_get_info(hd.h)["variant"] == 5) == (name == "n128")
+            check_chains(B, hd, orc, list(range(8)), 200, B.sa_get_trace(hd.h, 8, 200))
+        if name != "n128":
+            with Handle(B, prob, sched) as hd:
+                B.sa_select_kernel(hd.h, B.SA_KERNEL_DENSE)
+                with pytest.raises(B.SaError):
+                    B.sa_run(hd.h, 1)
 
 
 def test_extreme_tables(B, problems_cache):
