@@ -176,6 +176,8 @@ struct sa_handle {
   const uint32_t *d_init_frag = nullptr, *d_obs_word = nullptr, *d_fix = nullptr, *d_dwloc = nullptr, *d_dthloc = nullptr;
   const tsa::StaticKernel* dk = nullptr;
   bool dk_tried = false;
+  uint32_t* d_flags = nullptr;      // [R] hand-over flags of the balanced launch
+  int64_t last_slot_steps = 0;
   std::string dense_why;
   int family = SA_KERNEL_AUTO;
   std::string static_why;
@@ -325,6 +327,8 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->dplan.fix, &h->d_fix, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.wloc, &h->d_dwloc, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.thloc, &h->d_dthloc, st))) return rc;
+    h->d_flags = (uint32_t*)h->pool.alloc((size_t)sched->n_chains * 4, st);
+    if (!h->d_flags) return set_err(SA_ENOMEM, "device allocation failed (flags)");
   }
 
   const int R = sched->n_chains;
@@ -378,9 +382,22 @@ int sa_run(sa_handle* h, int64_t steps) {
   if (steps < 0) return set_err(SA_EINVAL, "steps < 0");
   if (steps == 0) return SA_OK;
   if (use_dense(h)) {
-    const tsa_dense::Params q = dense_params(h, steps);
     std::string why;
-    if (tsa::dense_kernel_launch(h->dk, (unsigned)h->C.R, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
+    tsa_dense::Params q = dense_params(h, steps);
+    unsigned grid = (unsigned)((h->C.R + h->dk->chains_per_cta - 1) / h->dk->chains_per_cta);
+    // More chains than resident slots: split the line of R*steps chain-steps evenly over the slots
+    // (DESIGN.md §6 "balanced slots") instead of running ceil(R / slots) uneven waves.
+    const int64_t slots = (int64_t)h->dk->blocks_per_sm * h->sm_count;
+    h->last_slot_steps = 0;
+    if (h->dk->chains_per_cta == 1 && slots > 0 && h->C.R > slots && !std::getenv("TSA_DENSE_NO_BALANCE")) {
+      const int64_t total = (int64_t)h->C.R * steps;
+      q.slot_steps = std::max<int64_t>((total + slots - 1) / slots, steps);
+      q.flags = h->d_flags;
+      TSA_CUDA(cudaMemsetAsync(h->d_flags, 0, (size_t)h->C.R * 4, h->stream));
+      grid = (unsigned)((total + q.slot_steps - 1) / q.slot_steps);
+      h->last_slot_steps = q.slot_steps;
+    }
+    if (tsa::dense_kernel_launch(h->dk, grid, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
     ++h->launches;
     h->g += (uint64_t)steps;
     return SA_OK;
@@ -643,9 +660,10 @@ int sa_get_info(sa_handle* h, int64_t info[16]) {
   if (h->dk && (env_family(h->family) == SA_KERNEL_AUTO || env_family(h->family) == SA_KERNEL_DENSE)) {
     info[0] = 5;                                 // dense kernel: one warp per chain, W in mma.sync A fragments
     info[1] = h->dk->threads;
-    info[2] = 1;
+    info[2] = h->dk->chains_per_cta;
     info[3] = (int64_t)h->dk->smem_bytes;
-    info[4] = h->C.R;
+    info[4] = (h->C.R + h->dk->chains_per_cta - 1) / h->dk->chains_per_cta;
+    if (h->last_slot_steps > 0) info[4] = (int64_t)h->dk->blocks_per_sm * h->sm_count;   // balanced slots
     info[14] = h->dk->regs;
     info[15] = h->dplan.W;
   }

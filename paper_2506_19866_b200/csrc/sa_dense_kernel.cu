@@ -33,7 +33,9 @@
 #define TSD_NPADA 128
 #define TSD_NFIX 1
 #define TSD_MINBLOCKS 8
-#define TSD_W 2
+#define TSD_W 1
+#define TSD_PH 1
+#define TSD_CPB 8
 #endif
 
 namespace tsa_dense {
@@ -41,17 +43,22 @@ namespace tsa_dense {
 constexpr int MT = TSD_MT, KS = TSD_KS, NW = TSD_KS, T = TSD_T, NOBS = TSD_NOBS;
 constexpr int CS = TSD_CS, TS = TSD_TS, NFIX = TSD_NFIX;
 constexpr int TW = TSD_W, TEAM = TW * 32;       // warps / threads per chain
+constexpr int CPB = TSD_CPB;                    // chains per CTA (one-warp chains only): 4 token rings of CPB/4 warps
 constexpr int WPW = NW / TW;                    // result words per condition a lane produces
 constexpr int MTW = 2 * WPW;                    // row tiles per warp (the last warp's may lie beyond MT)
+constexpr int PH = TSD_PH, WPP = WPW / PH;       // phases of a time step, result words per phase
 constexpr int NA = MTW * KS * 4;                // A-fragment registers per thread
 constexpr int STATE_BYTES = 8 * CS;             // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
+constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 2) * 4 + 15) / 16 * 16;   // bytes per chain
 constexpr u64 kObsLo = TSD_OBSMASK_LO, kObsHi = TSD_OBSMASK_HI;
 constexpr u32 kOnes = 0x01010101u, kTwos = 0x02020202u;
 constexpr bool kByteMism = NOBS * 2 * NW <= 255;   // mismatch counters stay in byte lanes
 static_assert(KS == 1 || KS == 2 || KS == 4, "KS must be 1, 2 or 4");
 static_assert(2 * KS >= MT && MT >= 1, "row <-> column numbering needs MT <= 2*KS");
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
+static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
+static_assert(CPB == 1 || (TW == 1 && CPB % 4 == 0 && CPB <= 12), "several chains per CTA: one-warp chains, whole rings, at most 15 named barriers");
 
 // Philox4x32-10 (Salmon et al., SC'11)
 __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1, u32 (&out)[4]) {
@@ -74,6 +81,10 @@ __device__ __forceinline__ u32 sign_mask(u32 x) {
 
 // D (16 x 8, s32) += A (16 x 32, s8, row) * B (32 x 8, s8, col)
 __device__ __forceinline__ void imma(int (&c)[4], const u32* a, u32 b0, u32 b1) {
+#ifdef TSD_PROBE_NO_IMMA      // timing probe only (wrong results): what the time step costs without the tensor pipe
+  c[0] += (int)(a[0] ^ b0); c[1] += (int)(a[1] ^ b1); c[2] += (int)a[2]; c[3] += (int)a[3];
+  return;
+#endif
   asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
@@ -96,6 +107,14 @@ __device__ __forceinline__ void sts_vec(u32 a, const u32 (&s)[4]) {
 }
 __device__ __forceinline__ void sts_u8(u32 a, u32 v) { asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
+// Tensor-pipe token ring.  Warps that share an SM sub-partition would otherwise fall into lock step
+// (all issue IMMAs together, then all do the integer work together, and the tensor pipe idles
+// half the time); instead the warp holding the token issues its IMMAs, passes the token on, and does
+// its integer work while the next warp uses the pipe.  One named barrier per warp, 64 threads:
+// the waiting warp's bar.sync and its predecessor's bar.arrive.
+__device__ __forceinline__ void ring_wait(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void ring_pass(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+
 // a[sel] ^= x for a run-time sel (a jump table: registers cannot be indexed); sel outside [0, NA) does nothing
 #define TSD_C1(i) case (i): if ((i) < NA) a[(i) < NA ? (i) : 0] ^= x; break;
 #define TSD_C4(i) TSD_C1(i) TSD_C1((i) + 1) TSD_C1((i) + 2) TSD_C1((i) + 3)
@@ -117,9 +136,61 @@ struct Regs {
   u32 fix[NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows)
 };
 
+// One phase of a time step: the IMMAs of the row tiles behind result words [P*WPP, (P+1)*WPP) of this
+// warp, then pack four sums to a word on top of the biased thresholds, compare, encode 0 / 1 / 2 per
+// byte, score against the observation words (a4) and store.  Phases run one after the other, so only
+// 2*WPP accumulator tiles are live at a time (the register budget that decides warps per SM).
+template <int P>
+struct Phases {
+  static __device__ __forceinline__ void run(const Regs& r, const u32 (&b)[2 * KS], int n_tiles, bool is_obs, const u32* ow,
+                                             u32& cnt, bool store, u32 st, int ring_me, int ring_next) {
+    constexpr int W0 = P * WPP;
+    int acc[2 * WPP][4];
+    if (CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
+#pragma unroll
+    for (int m = 0; m < 2 * WPP; ++m) { acc[m][0] = 0; acc[m][1] = 0; acc[m][2] = 0; acc[m][3] = 0; }
+#pragma unroll
+    for (int s = 0; s < KS; ++s)
+#pragma unroll
+      for (int mi = 0; mi < 2 * WPP; ++mi)
+        if (TW * MTW <= MT || 2 * W0 + mi < n_tiles) imma(acc[mi], &r.A[((2 * W0 + mi) * KS + s) * 4], b[2 * s], b[2 * s + 1]);
+    if (CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
+    u32 ns[2][WPP];
+#pragma unroll
+    for (int w = 0; w < WPP; ++w)
+#pragma unroll
+      for (int c = 0; c < 2; ++c) {
+        const u32 x = r.TA[W0 + w] + (u32)acc[2 * w][c] + ((u32)acc[2 * w][2 + c] << 8) + ((u32)acc[2 * w + 1][c] << 16) +
+                      ((u32)acc[2 * w + 1][2 + c] << 24);
+        const u32 ge = sign_mask(x);
+        const u32 gt = sign_mask(x + r.TD[W0 + w]);
+        ns[c][w] = ((ge ^ gt) & kOnes) | (gt & kTwos);
+      }
+    if (is_obs) {
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int w = 0; w < WPP; ++w) {
+          const u32 z = ns[c][w] ^ __ldg(ow + c * NW + W0 + w);
+          cnt += (z | (z >> 1)) & kOnes;
+        }
+    }
+    if (store) {
+      sts_vec(st + W0 * 4, ns[0]);
+      sts_vec(st + W0 * 4 + CS, ns[1]);
+    }
+    Phases<P + 1>::run(r, b, n_tiles, is_obs, ow, cnt, store, st, ring_me, ring_next);
+  }
+};
+template <>
+struct Phases<PH> {
+  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], int, bool, const u32*, u32&, bool, u32, int, int) {}
+};
+
 // a3 + a4 for the parameters now in registers: returns the team's mismatch count.
 // sbuf = shared address of the exchange buffer(s), red = the team's reduction words [2][TW].
-__device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf, volatile u32* red, int parity, int lane, int ww) {
+__device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf, volatile u32* red, int parity, int lane, int ww,
+                                        int ring_me, int ring_next) {
   const int g = lane >> 2, t4 = lane & 3;
   u32 st_addr = sbuf + (u32)((2 * t4) * CS + (g & 3) * TS + ((g >> 2) * NW + ww * WPW) * 4);
   u32 ld_addr = sbuf + (u32)(g * CS + t4 * TS);
@@ -135,45 +206,17 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
   int oj = 0;
 #pragma unroll 1
   for (int t = 1; t <= T; ++t) {
-    int acc[MTW][4];
-#pragma unroll
-    for (int m = 0; m < MTW; ++m) { acc[m][0] = 0; acc[m][1] = 0; acc[m][2] = 0; acc[m][3] = 0; }
-#pragma unroll
-    for (int s = 0; s < KS; ++s)
-#pragma unroll
-      for (int m = 0; m < MTW; ++m)
-        if (TW * MTW <= MT || m < n_tiles) imma(acc[m], &r.A[(m * KS + s) * 4], b[2 * s], b[2 * s + 1]);
-    // pack four sums to a word on top of the biased thresholds, compare, encode 0 / 1 / 2 per byte
-    u32 ns[2][WPW];
-#pragma unroll
-    for (int w = 0; w < WPW; ++w)
-#pragma unroll
-      for (int c = 0; c < 2; ++c) {
-        const u32 x = r.TA[w] + (u32)acc[2 * w][c] + ((u32)acc[2 * w][2 + c] << 8) + ((u32)acc[2 * w + 1][c] << 16) +
-                      ((u32)acc[2 * w + 1][2 + c] << 24);
-        const u32 ge = sign_mask(x);
-        const u32 gt = sign_mask(x + r.TD[w]);
-        ns[c][w] = ((ge ^ gt) & kOnes) | (gt & kTwos);
-      }
     const bool is_obs = t < 64 ? ((kObsLo >> t) & 1ull) : ((kObsHi >> (t - 64)) & 1ull);
+    const u32* ow = p.obs_word + ((size_t)oj * 32 + lane) * (2 * NW) + ww * WPW;
+    const u32 boff = NBUF == 2 ? (u32)(t & 1) * STATE_BYTES : 0u;
+    u32 cnt = 0u;                                         // per byte at most 2*WPW <= 8
+    if (TW == 1) __syncwarp();            // every lane has its B fragments out of the single buffer
+    Phases<0>::run(r, b, n_tiles, is_obs, ow, cnt, t < T, st_addr + boff, ring_me, ring_next);
     if (is_obs) {
-      const u32* ow = p.obs_word + ((size_t)oj * 32 + lane) * (2 * NW) + ww * WPW;
-      u32 cnt = 0u;                                       // per byte at most 2*WPW <= 8
-#pragma unroll
-      for (int c = 0; c < 2; ++c)
-#pragma unroll
-        for (int w = 0; w < WPW; ++w) {
-          const u32 z = ns[c][w] ^ __ldg(ow + c * NW + w);
-          cnt += (z | (z >> 1)) & kOnes;
-        }
       if (kByteMism) mis += cnt; else mis += __dp4a(cnt, kOnes, 0u);
       ++oj;
     }
     if (t < T) {
-      const u32 boff = NBUF == 2 ? (u32)(t & 1) * STATE_BYTES : 0u;
-      if (TW == 1) __syncwarp();          // every lane has its B fragments out of the single buffer
-      sts_vec(st_addr + boff, ns[0]);
-      sts_vec(st_addr + boff + CS, ns[1]);
       __syncwarp();
 #pragma unroll
       for (int f = 0; f < NFIX; ++f)
@@ -198,12 +241,97 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
   return (u32)((int)m + p.fit_const);
 }
 
-extern "C" __global__ void __launch_bounds__(TEAM, TSD_MINBLOCKS) tsa_run_dense(const __grid_constant__ Params p) {
-  extern __shared__ __align__(16) u32 smem[];
-  const int lane = threadIdx.x & 31, ww = threadIdx.x >> 5, g = lane >> 2, t4 = lane & 3;
-  const u32 chain = blockIdx.x;
+// a1: the proposal of step gs, as seen by this thread.
+struct Proposal {
+  u32 x2, pidx, loc, slot, wx;
+  int oldv, newv, wsel;
+  bool is_w, mine;
+};
+
+__device__ __forceinline__ Proposal propose(const Params& p, u64 gs, u32 gchain, int lane, int ww, int g, const i8* cw, const i8* cth) {
+  Proposal q;
+  u32 x[4];
+  philox4x32_10((u32)gs, (u32)(gs >> 32), gchain, 0u, p.key0, p.key1, x);
+  q.x2 = x[2];
+  q.pidx = __umulhi(x[0], (u32)TSD_NP);
+  q.is_w = q.pidx < (u32)TSD_NE;
+  q.loc = q.is_w ? __ldg(p.wloc + q.pidx) : __ldg(p.thloc + (q.pidx - (u32)TSD_NE));
+  q.slot = q.loc >> 16;
+  q.oldv = 0; q.newv = 0; q.wsel = -1; q.wx = 0u;
+  if (q.is_w) {
+    q.mine = ((q.loc >> 9) & 31u) == (u32)lane && ((q.loc >> 14) & 3u) == (u32)ww;
+    if (q.mine) {
+      q.oldv = cw[q.slot];
+      q.newv = (q.oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;      // (code + 1 + r) mod 3 - 1, code = old + 1
+      q.wsel = (int)(q.loc & 0x7Fu);
+      q.wx = ((u32)(q.oldv ^ q.newv) & 0xFFu) << (8 * ((q.loc >> 7) & 3u));
+    }
+  } else {
+    q.mine = (q.loc & 7u) == (u32)g && (int)((q.loc >> 3) & 3u) / WPW == ww;
+    if (q.mine) {
+      q.oldv = cth[q.slot];
+      q.newv = (q.oldv + 1 + (int)__umulhi(x[1], (u32)(TSD_NPAIRS - 1))) % TSD_NPAIRS;
+    }
+  }
+  return q;
+}
+
+// threshold bytes of the row at `loc` go from pair `from` to pair `to`
+__device__ __forceinline__ void shift_threshold(const Params& p, Regs& r, u32 loc, int from, int to) {
+  const int w = (int)((loc >> 3) & 3u) % WPW, sh = 8 * (int)((loc >> 5) & 3u);
+  const u32 da = (u32)((int)p.tha[to] - (int)p.tha[from]) << sh;
+  const u32 dd = (u32)(((int)p.tha[from] - (int)p.thb[from]) - ((int)p.tha[to] - (int)p.thb[to])) << sh;
+#pragma unroll
+  for (int i = 0; i < WPW; ++i) if (i == w) { r.TA[i] += da; r.TD[i] += dd; }
+}
+
+__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int ring_me, int ring_next);
+
+extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_dense(const __grid_constant__ Params p) {
+  extern __shared__ __align__(16) u32 smem_all[];
+  const int tix = threadIdx.x % TEAM, wc = threadIdx.x / TEAM;       // thread within the chain's team, chain slot within the CTA
+  const int lane = tix & 31, ww = tix >> 5, g = lane >> 2, t4 = lane & 3;
+  const u32 chain = blockIdx.x * CPB + wc;
+  // token ring of the CPB/4 one-warp chains that share this warp's SM sub-partition (warp wc, wc+4, ...):
+  // on only if every member has a chain; then all of them run the same number of time steps
+  int ring_me = 0, ring_next = 0;
+  if (CPB > 1) {
+    const int q = wc & 3, pos = wc >> 2, G = CPB / 4;
+    if (blockIdx.x * CPB + q + 4 * (G - 1) < (u32)p.R) {
+      ring_me = 1 + wc;
+      ring_next = 1 + q + 4 * ((pos + 1) % G);
+      if (pos == G - 1) ring_pass(ring_next);                        // the token starts at the ring's first warp
+    }
+    if (chain >= (u32)p.R) return;
+  }
+  u32* const smem = smem_all + (size_t)wc * (CHAIN_SMEM / 4);
+  if (p.slot_steps == 0) {
+    run_piece(p, chain, 0, p.steps, smem, tix, ring_me, ring_next);
+    return;
+  }
+  // balanced slots: this slot owns [lo, hi) of the line of R*steps chain-steps
+  const i64 S = p.steps, total = (i64)p.R * S;
+  const i64 lo = (i64)chain * p.slot_steps, hi = lo + p.slot_steps < total ? lo + p.slot_steps : total;
+  if (lo >= total) return;
+  const i64 ca = lo / S, cb = (hi - 1) / S, count = cb - ca + 1;
+  const bool head_first = cb > ca && hi < (cb + 1) * S;
+#pragma unroll 1
+  for (i64 n = 0; n < count; ++n) {
+    const i64 c = n == count - 1 ? ca : head_first ? (n == 0 ? cb : ca + n) : ca + 1 + n;
+    const i64 b0 = c * S;
+    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix, 0, 0);
+  }
+}
+
+// One piece of one chain's run: stage the chain (a0), advance it through steps [s0, s1) of this
+// launch, write it back (a7).  A launch normally gives every chain one piece, [0, steps); when there
+// are more chains than resident slots the host splits the (chain, step) line evenly over the slots
+// (slot_steps > 0), and a chain that straddles two slots is handed over through HBM: the slot that
+// runs its head does so FIRST and raises flags[chain]; the next slot runs the tail LAST.
+__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int ring_me, int ring_next) {
+  const int lane = tix & 31, ww = tix >> 5, g = lane >> 2, t4 = lane & 3;
   const u32 gchain = p.chain_id_base + chain;
-  // shared memory: exchange buffer(s), the chain's canonical weight and threshold rows, reduction words
+  // shared memory of this chain: exchange buffer(s), canonical weight and threshold rows, reduction and control words
   i8* const cw = (i8*)smem + NBUF * STATE_BYTES;
   i8* const cth = cw + TSD_EPADA;
   volatile u32* const red = (volatile u32*)(cth + TSD_NPADA);
@@ -213,10 +341,17 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSD_MINBLOCKS) tsa_run_dense(
   i8* const best_w = p.best_w + (size_t)chain * TSD_EPADA;
   i8* const best_th = p.best_th + (size_t)chain * TSD_NPADA;
 
+  if (s0 > 0) {                              // the head of this chain is another slot's first piece
+    if (tix == 0) {
+      while (*(volatile u32*)(p.flags + chain) == 0u) __nanosleep(200);
+      __threadfence();
+    }
+    team_sync();
+  }
   // a0: stage the chain
-  for (int x = threadIdx.x; x < NBUF * STATE_BYTES / 4; x += TEAM) smem[x] = 0u;
-  for (int x = threadIdx.x; x < TSD_EPADA / 4; x += TEAM) ((u32*)cw)[x] = ((const u32*)cur_w)[x];
-  for (int x = threadIdx.x; x < TSD_NPADA / 4; x += TEAM) ((u32*)cth)[x] = ((const u32*)cur_th)[x];
+  for (int x = tix; x < NBUF * STATE_BYTES / 4; x += TEAM) smem[x] = 0u;
+  for (int x = tix; x < TSD_EPADA / 4; x += TEAM) ((u32*)cw)[x] = __ldcg((const u32*)cur_w + x);
+  for (int x = tix; x < TSD_NPADA / 4; x += TEAM) ((u32*)cth)[x] = __ldcg((const u32*)cur_th + x);
   team_sync();
   Regs r;
 #pragma unroll
@@ -246,93 +381,74 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSD_MINBLOCKS) tsa_run_dense(
 #pragma unroll
   for (int f = 0; f < NFIX; ++f) r.fix[f] = __ldg(p.fix + (ww * NFIX + f) * 32 + lane);
 
-  u32 fcur = p.fit_cur[chain], fbest = p.fit_best[chain];
+  // Chain control words live in shared memory and the proposal is derived a second time after the
+  // simulation (from the step counter alone), so that nothing but the loop counter stays in
+  // registers across the time loop: the register budget there decides warps per SM.
+  volatile u32* const ctl = red + 2 * TW;               // [0] d_cur, [1] d_best
+  if (tix == 0) { ctl[0] = __ldcg(p.fit_cur + chain); ctl[1] = __ldcg(p.fit_best + chain); }
+  team_sync();
   const int trow = p.trace_row ? p.trace_row[chain] : -1;
-  u64 level = p.g0 / (u64)p.steps_per_level;
-  i64 left_in_level = p.steps_per_level - (i64)(p.g0 % (u64)p.steps_per_level);
 
 #pragma unroll 1
-  for (i64 it = 0; it < p.steps; ++it) {
-    const u64 gs = p.g0 + (u64)it;
-    u32 x[4];
-    philox4x32_10((u32)gs, (u32)(gs >> 32), gchain, 0u, p.key0, p.key1, x);
+  for (i64 it = s0; it < s1; ++it) {
     // a1 / a2: propose; the threads that hold the parameter apply it in their registers.  Only they
     // read or write its byte in the canonical row, so the row needs no barrier of its own.
-    const u32 pidx = __umulhi(x[0], (u32)TSD_NP);
-    const bool is_w = pidx < (u32)TSD_NE;
-    const u32 loc = is_w ? __ldg(p.wloc + pidx) : __ldg(p.thloc + (pidx - (u32)TSD_NE));
-    const u32 slot = loc >> 16;
-    int oldv = 0, newv = 0, wsel = -1;
-    u32 wx = 0u;
-    bool mine;
-    if (is_w) {
-      mine = ((loc >> 9) & 31u) == (u32)lane && ((loc >> 14) & 3u) == (u32)ww;
-      if (mine) {
-        oldv = cw[slot];
-        newv = (oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;          // (code + 1 + r) mod 3 - 1, code = old + 1
-        wsel = (int)(loc & 0x7Fu);
-        wx = ((u32)(oldv ^ newv) & 0xFFu) << (8 * ((loc >> 7) & 3u));
-      }
-      xor_reg(r.A, wsel, wx);
-    } else {
-      const int w = (int)((loc >> 3) & 3u);
-      mine = (loc & 7u) == (u32)g && w / WPW == ww;
-      if (mine) {
-        oldv = cth[slot];
-        newv = (oldv + 1 + (int)__umulhi(x[1], (u32)(TSD_NPAIRS - 1))) % TSD_NPAIRS;
-        const int sh = 8 * (int)((loc >> 5) & 3u);
-        const u32 da = (u32)((int)p.tha[newv] - (int)p.tha[oldv]) << sh;
-        const u32 dd = (u32)(((int)p.tha[oldv] - (int)p.thb[oldv]) - ((int)p.tha[newv] - (int)p.thb[newv])) << sh;
-#pragma unroll
-        for (int i = 0; i < WPW; ++i) if (i == w % WPW) { r.TA[i] += da; r.TD[i] += dd; }
-      }
+    {
+      const Proposal q = propose(p, p.g0 + (u64)it, gchain, lane, ww, g, cw, cth);
+      if (q.is_w) xor_reg(r.A, q.wsel, q.wx);
+      else if (q.mine) shift_threshold(p, r, q.loc, q.oldv, q.newv);
     }
     // a3 / a4
-    const u32 fcand = simulate(p, r, sbuf, red, (int)(it & 1), lane, ww);
+    const u32 fcand = simulate(p, r, sbuf, red, (int)(it & 1), lane, ww, ring_me, ring_next);
     // a5
-    const u64 lv = level < (u64)(p.n_levels - 1) ? level : (u64)(p.n_levels - 1);
+    u64 gs = p.g0 + (u64)it;
+    asm volatile("" : "+l"(gs));                         // opaque: derive the proposal again instead of keeping it live
+    const Proposal q = propose(p, gs, gchain, lane, ww, g, cw, cth);
+    const u32 fcur = ctl[0], fbest = ctl[1];
+    u64 level = ((gs | (u64)p.steps_per_level) >> 32) == 0 ? (u64)((u32)gs / (u32)p.steps_per_level) : gs / (u64)p.steps_per_level;
+    if (level > (u64)(p.n_levels - 1)) level = (u64)(p.n_levels - 1);
     const i64 d = (i64)fcand - (i64)fcur;
     bool acc = d <= 0;
-    if (!acc && d <= (i64)p.dmax) acc = x[2] < __ldg(p.accept + lv * (u64)p.dmax + (u64)(d - 1));
-    bool new_best = false;
+    if (!acc && d <= (i64)p.dmax) acc = q.x2 < __ldg(p.accept + level * (u64)p.dmax + (u64)(d - 1));
+    const bool new_best = acc && fcand < fbest;
+    team_sync();                                         // everyone has read the control words
     // a6
     if (acc) {
-      fcur = fcand;
-      if (mine) {
-        if (is_w) cw[slot] = (i8)newv;
-        else if (t4 == 0) cth[slot] = (i8)newv;
+      if (tix == 0) { ctl[0] = fcand; if (new_best) ctl[1] = fcand; }
+      if (q.mine) {
+        if (q.is_w) cw[q.slot] = (i8)q.newv;
+        else if (t4 == 0) cth[q.slot] = (i8)q.newv;
       }
-      if (fcand < fbest) {
-        fbest = fcand;
-        new_best = true;
+      if (new_best) {
         team_sync();
-        for (int i = threadIdx.x; i < TSD_EPADA / 4; i += TEAM) ((u32*)best_w)[i] = ((const u32*)cw)[i];
-        for (int i = threadIdx.x; i < TSD_NPADA / 4; i += TEAM) ((u32*)best_th)[i] = ((const u32*)cth)[i];
+        for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)best_w)[i] = ((const u32*)cw)[i];
+        for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)best_th)[i] = ((const u32*)cth)[i];
       }
-    } else if (is_w) {
-      xor_reg(r.A, wsel, wx);
-    } else if (mine) {
-      const int w = (int)((loc >> 3) & 3u), sh = 8 * (int)((loc >> 5) & 3u);
-      const u32 da = (u32)((int)p.tha[oldv] - (int)p.tha[newv]) << sh;
-      const u32 dd = (u32)(((int)p.tha[newv] - (int)p.thb[newv]) - ((int)p.tha[oldv] - (int)p.thb[oldv])) << sh;
-#pragma unroll
-      for (int i = 0; i < WPW; ++i) if (i == w % WPW) { r.TA[i] += da; r.TD[i] += dd; }
+    } else if (q.is_w) {
+      xor_reg(r.A, q.wsel, q.wx);
+    } else if (q.mine) {
+      shift_threshold(p, r, q.loc, q.newv, q.oldv);
     }
-    __syncwarp();
-    if (trow >= 0 && mine && (is_w || t4 == 0)) {
+    team_sync();
+    if (trow >= 0 && q.mine && (q.is_w || t4 == 0)) {
       const u64 idx = gs - p.trace_g0;
-      const u32 code = is_w ? (u32)(newv + 1) : (u32)newv;
+      const u32 code = q.is_w ? (u32)(q.newv + 1) : (u32)q.newv;
       if (gs >= p.trace_g0 && idx < (u64)p.trace_max)
         p.trace_rec[(size_t)trow * (size_t)p.trace_max + idx] =
-            (u64)fcand | ((u64)pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61);
+            (u64)fcand | ((u64)q.pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61);
     }
-    if (--left_in_level == 0) { ++level; left_in_level = p.steps_per_level; }
   }
   // a7
   team_sync();
-  for (int i = threadIdx.x; i < TSD_EPADA / 4; i += TEAM) ((u32*)cur_w)[i] = ((const u32*)cw)[i];
-  for (int i = threadIdx.x; i < TSD_NPADA / 4; i += TEAM) ((u32*)cur_th)[i] = ((const u32*)cth)[i];
-  if (threadIdx.x == 0) { p.fit_cur[chain] = fcur; p.fit_best[chain] = fbest; }
+  for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)cur_w)[i] = ((const u32*)cw)[i];
+  for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)cur_th)[i] = ((const u32*)cth)[i];
+  if (tix == 0) { p.fit_cur[chain] = ctl[0]; p.fit_best[chain] = ctl[1]; }
+  if (s1 < p.steps) {                        // hand the chain over
+    __threadfence();
+    team_sync();
+    if (tix == 0) { __threadfence(); atomicExch(p.flags + chain, 1u); }
+  }
+  team_sync();                               // the shared memory is free for the next piece
 }
 
 }  // namespace tsa_dense

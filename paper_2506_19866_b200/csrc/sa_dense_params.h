@@ -49,6 +49,10 @@ struct Params {
   // this launch
   u64 g0;
   i64 steps;
+  // balanced slots (0 = one chain per slot): every slot advances slot_steps chain-steps of the line
+  // of R*steps; flags[chain] != 0 once the head piece of a straddling chain is back in HBM
+  i64 slot_steps;
+  u32* flags;             // [R], zeroed by the host before the launch
 };
 
 }  // namespace tsa_dense

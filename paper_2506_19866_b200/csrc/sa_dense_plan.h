@@ -27,8 +27,8 @@ struct DensePlan {
   std::vector<uint32_t> fix;         // [W][n_fix_rounds][32]
   std::vector<uint32_t> wloc;        // [E]
   std::vector<uint32_t> thloc;       // [N]
-  size_t smem_bytes(const Plan& pl) const {
-    return (size_t)(W > 1 ? 2 : 1) * 8 * CS + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)2 * W * 4;
+  size_t smem_bytes(const Plan& pl) const {   // per chain, as CHAIN_SMEM in the kernel
+    return ((size_t)(W > 1 ? 2 : 1) * 8 * CS + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 2) * 4 + 15) / 16 * 16;
   }
 };
 

@@ -18,7 +18,9 @@ struct StaticTuning {
   int max_regs = 128;     // register budget per thread -> __launch_bounds__ min blocks
   int batch = 8;          // state gathers issued back to back before their IMADs
   int t_unroll = 1;       // unroll factor of the time loop
-  int dense_blocks = 8;   // dense kernel: resident chains (CTAs) per SM the register allocation aims at
+  int dense_blocks = 12;  // dense kernel: resident chains (CTAs) per SM the register allocation aims at (12 -> 168 registers)
+  int dense_phases = 1;   // dense kernel: phases of a time step (accumulator tiles live at a time = row tiles / phases)
+  int dense_cpb = 1;      // dense kernel: one-warp chains per CTA (1, 4, 8 or 12); > 1 turns the tensor-pipe token ring on
   int dense_warps = 1;    // dense kernel: warps per chain (1, 2 or 4); 1 measured fastest at every R
   static StaticTuning from_env();
 };
@@ -30,6 +32,8 @@ std::vector<std::string> static_kernel_defines(const Plan& plan, const StaticTun
 bool static_kernel_compile(const std::vector<std::string>& defines, std::string* cubin, std::string* log);
 
 struct StaticKernel {
+  int chains_per_cta = 1;
+  int blocks_per_sm = 0;      // resident CTAs per SM at this kernel's registers and shared memory (occupancy query)
   void* module = nullptr;     // CUmodule
   void* function = nullptr;   // CUfunction
   int threads = 0;
@@ -47,6 +51,8 @@ int static_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, con
 // The dense (tensor-pipe) kernel, sa_dense_kernel.cu: same cache, loader and launch path.
 std::vector<std::string> dense_kernel_defines(const Plan& plan, const DensePlan& dp, const StaticTuning& tune);
 bool dense_kernel_compile(const std::vector<std::string>& defines, std::string* cubin, std::string* log);
+// chains per CTA the kernel will be built for (1 unless the plan has one-warp chains)
+int dense_chains_per_cta(const DensePlan& dp, const StaticTuning& tune);
 const StaticKernel* dense_kernel_get(const Plan& plan, const DensePlan& dp, const StaticTuning& tune, std::string* why);
 int dense_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_dense::Params& params, std::string* why);
 

@@ -279,6 +279,36 @@ def test_every_kernel_family_matches_the_oracle(B, problems_cache, name, family,
             del os.environ[k]
 
 
+def test_balanced_slots_hand_chains_over(B, problems_cache):
+    """More chains than resident slots: the dense kernel splits the line of R*steps chain-steps evenly
+    over the slots and hands straddling chains from one slot to the next through HBM.  Results are
+    those of the plain launch and of the oracle; two sa_run calls cut the line at different places."""
+    prob = problems_cache("mtb")
+    orc = O.Oracle(prob)
+    R, steps = 2600, 44
+    sched = PB.default_schedule("mtb", n_chains=R, total_steps=steps)
+    chains = sorted(set(list(range(0, R, 113)) + [1, 2, 3, R - 2, R - 1]))
+    with Handle(B, prob, sched) as hd:
+        B.sa_select_kernel(hd.h, B.SA_KERNEL_DENSE)
+        B.sa_set_trace(hd.h, chains, steps)
+        B.sa_run(hd.h, 17)
+        B.sa_run(hd.h, steps - 17)
+        info = B.sa_get_info(hd.h)
+        assert info["variant"] == 5 and info["grid"] < R, info
+        check_chains(B, hd, orc, chains, steps, B.sa_get_trace(hd.h, len(chains), steps))
+        balanced = B.sa_get_fitness(hd.h, R)
+    os.environ["TSA_DENSE_NO_BALANCE"] = "1"
+    try:
+        with Handle(B, prob, sched) as hd:
+            B.sa_select_kernel(hd.h, B.SA_KERNEL_DENSE)
+            B.sa_run(hd.h, steps)
+            assert B.sa_get_info(hd.h)["grid"] == R
+            plain = B.sa_get_fitness(hd.h, R)
+    finally:
+        del os.environ["TSA_DENSE_NO_BALANCE"]
+    assert np.array_equal(balanced[0], plain[0]) and np.array_equal(balanced[1], plain[1])
+
+
 def test_dense_kernel_limits(B):
     """The dense family applies up to 128 nodes and 8 conditions; beyond that DENSE fails loudly
     and AUTO falls back to the gather kernels with identical results."""
