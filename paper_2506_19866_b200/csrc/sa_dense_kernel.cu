@@ -220,7 +220,7 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
       __syncwarp();
 #pragma unroll
       for (int f = 0; f < NFIX; ++f)
-        if (r.fix[f] >> 31) sts_u8(sbuf + boff + (r.fix[f] & 0xFFFFu), (r.fix[f] >> 16) & 3u);
+        if (r.fix[f] >> 31) sts_u8((r.fix[f] & 0xFFFFFFu) + boff, (r.fix[f] >> 24) & 3u);
       team_sync();
       u32 lo[NW], hi[NW];
       lds_vec(ld_addr + boff, lo);
@@ -290,7 +290,6 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
 extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_dense(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) u32 smem_all[];
   const int tix = threadIdx.x % TEAM, wc = threadIdx.x / TEAM;       // thread within the chain's team, chain slot within the CTA
-  const int lane = tix & 31, ww = tix >> 5, g = lane >> 2, t4 = lane & 3;
   const u32 chain = blockIdx.x * CPB + wc;
   // token ring of the CPB/4 one-warp chains that share this warp's SM sub-partition (warp wc, wc+4, ...):
   // on only if every member has a chain; then all of them run the same number of time steps
@@ -305,21 +304,25 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
     if (chain >= (u32)p.R) return;
   }
   u32* const smem = smem_all + (size_t)wc * (CHAIN_SMEM / 4);
-  if (p.slot_steps == 0) {
-    run_piece(p, chain, 0, p.steps, smem, tix, ring_me, ring_next);
-    return;
-  }
-  // balanced slots: this slot owns [lo, hi) of the line of R*steps chain-steps
-  const i64 S = p.steps, total = (i64)p.R * S;
-  const i64 lo = (i64)chain * p.slot_steps, hi = lo + p.slot_steps < total ? lo + p.slot_steps : total;
-  if (lo >= total) return;
-  const i64 ca = lo / S, cb = (hi - 1) / S, count = cb - ca + 1;
-  const bool head_first = cb > ca && hi < (cb + 1) * S;
+  // one chain per slot (slot_steps == 0), or balanced slots: this slot owns [lo, hi) of the line of
+  // R*steps chain-steps and visits the chains ca .. cb it touches, one piece each
+  // (the slot's bounds are derived again for every piece, from an opaque copy of the slot index, so
+  // that they do not occupy registers across the time loop)
 #pragma unroll 1
-  for (i64 n = 0; n < count; ++n) {
+  for (int n = 0;; ++n) {
+    u32 slot = chain;
+    asm volatile("" : "+r"(slot));
+    const i64 S = p.steps, total = (i64)p.R * S;
+    const i64 lo = p.slot_steps == 0 ? (i64)slot * S : (i64)slot * p.slot_steps;
+    const i64 hi = p.slot_steps == 0 ? lo + S : (lo + p.slot_steps < total ? lo + p.slot_steps : total);
+    if (lo >= total) return;
+    const i64 ca = lo / S, cb = (hi - 1) / S;
+    const int count = (int)(cb - ca) + 1;
+    if (n >= count) return;
+    const bool head_first = cb > ca && hi < (cb + 1) * S;
     const i64 c = n == count - 1 ? ca : head_first ? (n == 0 ? cb : ca + n) : ca + 1 + n;
     const i64 b0 = c * S;
-    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix, 0, 0);
+    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix, ring_me, ring_next);
   }
 }
 
@@ -336,10 +339,7 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   i8* const cth = cw + TSD_EPADA;
   volatile u32* const red = (volatile u32*)(cth + TSD_NPADA);
   const u32 sbuf = (u32)__cvta_generic_to_shared(smem);
-  i8* const cur_w = p.cur_w + (size_t)chain * TSD_EPADA;
-  i8* const cur_th = p.cur_th + (size_t)chain * TSD_NPADA;
-  i8* const best_w = p.best_w + (size_t)chain * TSD_EPADA;
-  i8* const best_th = p.best_th + (size_t)chain * TSD_NPADA;
+  // (row addresses are formed where they are used, never held across the time loop)
 
   if (s0 > 0) {                              // the head of this chain is another slot's first piece
     if (tix == 0) {
@@ -350,8 +350,8 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   }
   // a0: stage the chain
   for (int x = tix; x < NBUF * STATE_BYTES / 4; x += TEAM) smem[x] = 0u;
-  for (int x = tix; x < TSD_EPADA / 4; x += TEAM) ((u32*)cw)[x] = __ldcg((const u32*)cur_w + x);
-  for (int x = tix; x < TSD_NPADA / 4; x += TEAM) ((u32*)cth)[x] = __ldcg((const u32*)cur_th + x);
+  for (int x = tix; x < TSD_EPADA / 4; x += TEAM) ((u32*)cw)[x] = __ldcg((const u32*)(p.cur_w + (size_t)chain * TSD_EPADA) + x);
+  for (int x = tix; x < TSD_NPADA / 4; x += TEAM) ((u32*)cth)[x] = __ldcg((const u32*)(p.cur_th + (size_t)chain * TSD_NPADA) + x);
   team_sync();
   Regs r;
 #pragma unroll
@@ -379,7 +379,10 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     r.TA[w] = ta; r.TD[w] = td;
   }
 #pragma unroll
-  for (int f = 0; f < NFIX; ++f) r.fix[f] = __ldg(p.fix + (ww * NFIX + f) * 32 + lane);
+  for (int f = 0; f < NFIX; ++f) {                      // bit 31 valid, 24-25 value, 0-23 shared address of the byte
+    const u32 raw = __ldg(p.fix + (ww * NFIX + f) * 32 + lane);
+    r.fix[f] = (raw & 0x80000000u) | (((raw >> 16) & 3u) << 24) | (sbuf + (raw & 0xFFFFu));
+  }
 
   // Chain control words live in shared memory and the proposal is derived a second time after the
   // simulation (from the step counter alone), so that nothing but the loop counter stays in
@@ -387,7 +390,6 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   volatile u32* const ctl = red + 2 * TW;               // [0] d_cur, [1] d_best
   if (tix == 0) { ctl[0] = __ldcg(p.fit_cur + chain); ctl[1] = __ldcg(p.fit_best + chain); }
   team_sync();
-  const int trow = p.trace_row ? p.trace_row[chain] : -1;
 
 #pragma unroll 1
   for (i64 it = s0; it < s1; ++it) {
@@ -421,8 +423,10 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
       }
       if (new_best) {
         team_sync();
-        for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)best_w)[i] = ((const u32*)cw)[i];
-        for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)best_th)[i] = ((const u32*)cth)[i];
+        u32* const best_w = (u32*)(p.best_w + (size_t)chain * TSD_EPADA);
+        u32* const best_th = (u32*)(p.best_th + (size_t)chain * TSD_NPADA);
+        for (int i = tix; i < TSD_EPADA / 4; i += TEAM) best_w[i] = ((const u32*)cw)[i];
+        for (int i = tix; i < TSD_NPADA / 4; i += TEAM) best_th[i] = ((const u32*)cth)[i];
       }
     } else if (q.is_w) {
       xor_reg(r.A, q.wsel, q.wx);
@@ -430,6 +434,7 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
       shift_threshold(p, r, q.loc, q.newv, q.oldv);
     }
     team_sync();
+    const int trow = p.trace_row ? __ldg(p.trace_row + chain) : -1;
     if (trow >= 0 && q.mine && (q.is_w || t4 == 0)) {
       const u64 idx = gs - p.trace_g0;
       const u32 code = q.is_w ? (u32)(q.newv + 1) : (u32)q.newv;
@@ -440,8 +445,8 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   }
   // a7
   team_sync();
-  for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)cur_w)[i] = ((const u32*)cw)[i];
-  for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)cur_th)[i] = ((const u32*)cth)[i];
+  for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)(p.cur_w + (size_t)chain * TSD_EPADA))[i] = ((const u32*)cw)[i];
+  for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)(p.cur_th + (size_t)chain * TSD_NPADA))[i] = ((const u32*)cth)[i];
   if (tix == 0) { p.fit_cur[chain] = ctl[0]; p.fit_best[chain] = ctl[1]; }
   if (s1 < p.steps) {                        // hand the chain over
     __threadfence();
