@@ -98,6 +98,20 @@ def _workload(name: str, args):
     return spec, chains, sa_steps
 
 
+def rank_chain_base(rank: int, chains_per_gpu: int) -> int:
+    """Chain-range partition: rank r owns global chains [r*R, (r+1)*R) (reading 25)."""
+    return rank * chains_per_gpu
+
+
+def max_over_ranks(ms: float, dist, device="cuda") -> float:
+    """Device time of the slowest rank (the job's time); dist = torch.distributed or None."""
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 # ------------------------------------------------------------------------------------ ours
 def run_ours(args) -> dict:
     import torch
@@ -125,7 +139,7 @@ def run_ours(args) -> dict:
         # inputs: synthetic, seeded; the ground-truth time courses come from the library's own
         # sa_simulate (the oracle is not on this path)
         prob = PB.make_problem(name, B.sa_simulate)
-        sched = PB.make_schedule(chains, sa_steps, chain_id_base=rank * chains)
+        sched = PB.make_schedule(chains, sa_steps, chain_id_base=rank_chain_base(rank, chains))
         flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")   # > 126 MB L2
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         info = None
@@ -147,10 +161,7 @@ def run_ours(args) -> dict:
             B.sa_destroy(h)
         ms = [a.elapsed_time(b) for a, b in ev]
         kernel_ms = sum(ms)
-        total_ms = torch.tensor([kernel_ms], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-        total_ms = float(total_ms.item())
+        total_ms = max_over_ranks(kernel_ms, dist)
         res = {"prob": prob, "sched": sched, "ms": ms, "total_ms": total_ms, "info": info, "best": best,
                "chain_steps": chains * sa_steps * steps * world}
         if want_e2e:

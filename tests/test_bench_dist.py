@@ -1,0 +1,72 @@
+"""The N > 1 plumbing of bench.py on CPU (gloo, world size 2): chain-range partition by rank,
+max-over-ranks timing, rank 0 alone reports.  The data path has no collective."""
+import json
+import os
+import subprocess
+import sys
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+WORKER = r"""
+import json, os, sys
+sys.path.insert(0, {root!r})
+import numpy as np
+import torch
+import torch.distributed as dist
+import bench
+from oracle import oracle as O
+from paper_2506_19866_b200 import problems as PB
+
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+chains = 3
+prob = PB.make_problem("tiny", O.simulate_fn)
+sched = PB.make_schedule(chains, 200, chain_id_base=bench.rank_chain_base(rank, chains))
+orc = O.Oracle(prob)
+fits = [orc.run_chain(sched, c + sched.chain_id_base, 200)["fit_best"] for c in range(chains)]
+mine = torch.tensor(fits, dtype=torch.int64)
+gathered = [torch.zeros_like(mine) for _ in range(world)]
+dist.all_gather(gathered, mine)
+ms = bench.max_over_ranks(10.0 + 5.0 * rank, dist, device="cpu")
+if rank == 0:
+    print(json.dumps({{"fits": torch.cat(gathered).tolist(), "ms": ms, "world": world}}))
+dist.barrier()
+dist.destroy_process_group()
+"""
+
+
+def test_two_rank_partition_and_timing(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(WORKER.format(root=ROOT))
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29671", str(script)],
+                         capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
+    got = json.loads(line)
+    assert got["world"] == 2 and got["ms"] == 15.0          # the slowest rank sets the time
+    # the two ranks' chains are global chains 0..5 of one 6-chain run
+    sys.path.insert(0, ROOT)
+    from oracle import oracle as O
+    from paper_2506_19866_b200 import problems as PB
+    prob = PB.make_problem("tiny", O.simulate_fn)
+    sched = PB.make_schedule(6, 200)
+    orc = O.Oracle(prob)
+    ref = [orc.run_chain(sched, c, 200)["fit_best"] for c in range(6)]
+    assert got["fits"] == ref
+
+
+def test_reference_arm_prints_on_rank0_only():
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1")
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29672", os.path.join(ROOT, "bench.py"),
+                          "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0", "--workload", "tiny"],
+                         capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
