@@ -201,7 +201,13 @@ bool use_dense(sa_handle* h) {
   if (fam != SA_KERNEL_AUTO && fam != SA_KERNEL_DENSE) return false;
   if (!h->dk_tried) {
     h->dk_tried = true;
-    h->dk = tsa::dense_kernel_get(h->plan, h->dplan, tsa::StaticTuning::from_env(), &h->dense_why);
+    tsa::StaticTuning tune = tsa::StaticTuning::from_env();
+    if (!std::getenv("TSA_DENSE_BLOCKS")) {
+      // fewer chains than slots: do not squeeze the registers for an occupancy the grid cannot reach
+      const int per_sm = (int)((h->C.R + h->sm_count - 1) / std::max(h->sm_count, 1));
+      tune.dense_blocks = std::max(1, std::min(tune.dense_blocks, per_sm));
+    }
+    h->dk = tsa::dense_kernel_get(h->plan, h->dplan, tune, &h->dense_why);
   }
   return h->dk != nullptr;
 }

@@ -36,6 +36,7 @@
 #define TSD_W 1
 #define TSD_PH 1
 #define TSD_CPB 8
+#define TSD_REDERIVE 1
 #endif
 
 namespace tsa_dense {
@@ -43,6 +44,7 @@ namespace tsa_dense {
 constexpr int MT = TSD_MT, KS = TSD_KS, NW = TSD_KS, T = TSD_T, NOBS = TSD_NOBS;
 constexpr int CS = TSD_CS, TS = TSD_TS, NFIX = TSD_NFIX;
 constexpr int TW = TSD_W, TEAM = TW * 32;       // warps / threads per chain
+constexpr bool REDERIVE = TSD_REDERIVE != 0;    // tight register budget: derive the proposal twice rather than hold it over the time loop
 constexpr int CPB = TSD_CPB;                    // chains per CTA (one-warp chains only): 4 token rings of CPB/4 warps
 constexpr int WPW = NW / TW;                    // result words per condition a lane produces
 constexpr int MTW = 2 * WPW;                    // row tiles per warp (the last warp's may lie beyond MT)
@@ -395,17 +397,15 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   for (i64 it = s0; it < s1; ++it) {
     // a1 / a2: propose; the threads that hold the parameter apply it in their registers.  Only they
     // read or write its byte in the canonical row, so the row needs no barrier of its own.
-    {
-      const Proposal q = propose(p, p.g0 + (u64)it, gchain, lane, ww, g, cw, cth);
-      if (q.is_w) xor_reg(r.A, q.wsel, q.wx);
-      else if (q.mine) shift_threshold(p, r, q.loc, q.oldv, q.newv);
-    }
+    const Proposal q1 = propose(p, p.g0 + (u64)it, gchain, lane, ww, g, cw, cth);
+    if (q1.is_w) xor_reg(r.A, q1.wsel, q1.wx);
+    else if (q1.mine) shift_threshold(p, r, q1.loc, q1.oldv, q1.newv);
     // a3 / a4
     const u32 fcand = simulate(p, r, sbuf, red, (int)(it & 1), lane, ww, ring_me, ring_next);
     // a5
     u64 gs = p.g0 + (u64)it;
-    asm volatile("" : "+l"(gs));                         // opaque: derive the proposal again instead of keeping it live
-    const Proposal q = propose(p, gs, gchain, lane, ww, g, cw, cth);
+    if (REDERIVE) asm volatile("" : "+l"(gs));           // opaque: derive the proposal again instead of keeping it live
+    const Proposal q = REDERIVE ? propose(p, gs, gchain, lane, ww, g, cw, cth) : q1;
     const u32 fcur = ctl[0], fbest = ctl[1];
     u64 level = ((gs | (u64)p.steps_per_level) >> 32) == 0 ? (u64)((u32)gs / (u32)p.steps_per_level) : gs / (u64)p.steps_per_level;
     if (level > (u64)(p.n_levels - 1)) level = (u64)(p.n_levels - 1);
