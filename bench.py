@@ -204,7 +204,7 @@ def run_ours(args) -> dict:
         out = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": main["total_ms"] / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "int8/int32 (SWAR byte lanes)", "data": "synthetic",
+            "scaling": "weak", "vs_baseline": None, "dtype": "int8 (mma.sync s8 x s8 -> s32, byte-lane SWAR thresholds)", "data": "synthetic",
             "config": {"workload": f"{name}-shaped: N={prob.n_nodes} E={prob.n_edges} K={prob.n_cond} "
                                    f"T={prob.n_steps} n_obs={prob.n_obs}, R={chains} chains/GPU x {sa_steps} SA steps",
                        "chains_per_gpu": chains, "sa_steps": sa_steps, "seed": prob.seed, "sa_seed": PB.SA_SEED,
@@ -216,11 +216,22 @@ def run_ours(args) -> dict:
             "gpu_launches": args.steps,
             "e2e": main["e2e"], "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
-                         "unit": "T int-lane-op/s", "frac": achieved / issue_peak, "traffic": None,
+                         "unit": "T int-lane-op/s", "frac": achieved / issue_peak,
+                         # dram__bytes_read.sum + dram__bytes_write.sum of one sa_run launch, from the ncu capture in
+                         # profiles/r1_v4_run_dense_kernel.md (stage + write back of the chains; HBM is not the bound)
+                         "traffic": 6.16e6 if name == "mtb" else None,
                          "peak_source": f"{sms} SMs x 4 schedulers x 32 lanes x {sm_max_hz/1e6:.0f} MHz "
                                         "(MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §7)",
                          "alg_ops_per_chain_step": prob.alg_ops_per_step},
         }
+        if main["info"]["variant"] == 5:
+            # second ceiling of the dense kernel: MT*KS IMMA.16832.S8 per time step against the measured
+            # 0.5 IMMA per clock per SM of the legacy tensor path on B200
+            mt = (prob.n_nodes + 15) // 16
+            ks = {1: 1, 2: 2, 3: 4, 4: 4}[(mt + 1) // 2]
+            immas = prob.n_steps * mt * ks * chains * sa_steps / kernel_s
+            out["roofline"]["tensor_pipe"] = {"imma_per_chain_step": prob.n_steps * mt * ks, "achieved_imma_per_s": immas,
+                                              "peak_imma_per_s": 0.5 * sms * sm_max_hz, "frac": immas / (0.5 * sms * sm_max_hz)}
         if world == 1 and not args.no_extra:
             try:
                 pk = B.sa_int32_peak()

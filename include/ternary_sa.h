@@ -123,8 +123,10 @@ int sa_geometric_table(double t0, double t_end, int32_t n_levels, int32_t dmax, 
  * memory bytes per CTA, [4] = CTAs in the sa_run grid, [5] = edge slots per chain (padded),
  * [6] = SM count, [7] = kernels launched so far by this handle, [8] = passes per time step,
  * [9] = edge iterations per time step (sum over passes), [10] = rows, [11] = split nodes,
- * [12] = state words per node, [13] = state entries, [14] = registers per thread of the static
- * kernel (0 if not loaded), [15] = warps per chain of the static schedule (0 = not applicable).
+ * [12] = state words per node, [13] = state entries, [14] = registers per thread of the static /
+ * dense kernel (0 if not loaded), [15] = warps per chain of the static schedule or the dense team
+ * (0 = not applicable).  For the dense kernel [4] is the number of resident slots when the last
+ * sa_run used balanced slots (more chains than slots).
  * The variant is decided at the first sa_run; before it, info[0] reports the generic choice. */
 int sa_get_info(sa_handle *h, int64_t info[16]);
 

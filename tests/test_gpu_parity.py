@@ -248,11 +248,13 @@ FAMILY_CASES = [
     ("hpg", "GENERIC", {}), ("hpg", "STATIC", {}), ("hpg", "DENSE", {}),
     ("mtb", "GENERIC", {}), ("mtb", "STATIC", {}), ("mtb", "DENSE", {}),
     ("mtb", "DENSE", {"TSA_DENSE_W": "2"}), ("mtb", "DENSE", {"TSA_DENSE_W": "4"}),
-    ("mtb", "DENSE", {"TSA_DENSE_BLOCKS": "12"}),
+    ("mtb", "DENSE", {"TSA_DENSE_BLOCKS": "8"}), ("mtb", "DENSE", {"TSA_DENSE_PH": "2"}),
+    ("mtb", "DENSE", {"TSA_DENSE_CPB": "8"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "12"}),
+    ("hpg", "DENSE", {"TSA_DENSE_CPB": "4"}),
 ]
 
 
-@pytest.mark.parametrize("name,family,env", FAMILY_CASES, ids=[f"{n}-{f}-{'-'.join(e.values()) or 'default'}" for n, f, e in FAMILY_CASES])
+@pytest.mark.parametrize("name,family,env", FAMILY_CASES, ids=[f"{n}-{f}-{'-'.join(k[10:] + v for k, v in e.items()) or 'default'}" for n, f, e in FAMILY_CASES])
 def test_every_kernel_family_matches_the_oracle(B, problems_cache, name, family, env):
     """sa_run has three kernel families (include/ternary_sa.h); each one, forced, reproduces the
     oracle's trace, vectors and fitness, and says which one ran."""
