@@ -98,6 +98,14 @@ int sa_eval(sa_handle *h, const int8_t *params, int64_t n, uint32_t *fitness);
  * series).  Needs no handle; obs->obs is ignored and may be NULL. */
 int sa_simulate(const sa_network *net, const sa_observations *obs, const int8_t *params, uint8_t *states);
 
+/* The level structure of PAPER.md Table 1 (:125-155) with the synchronisation done on the device:
+ * n_levels times { sa_run(steps_per_level); then, per group of group_size consecutive chains, the
+ * member with the smallest best fitness (ties: smallest chain) gives its best vector to every member
+ * as best AND current vector, fitness included }.  group_size = 0: all chains form one group (the
+ * paper's algorithm); 32 is the group-wise variant of its future work (:321).  The step counter must
+ * be at a level boundary.  Asynchronous like sa_run; the synchronisation is not traced. */
+int sa_run_levels(sa_handle *h, int64_t n_levels, int32_t group_size);
+
 /* One chain's current and best vectors ([E+N] each) and fitnesses.  Any output may be NULL. */
 int sa_get_chain(sa_handle *h, int32_t chain, int8_t *cur, uint32_t *cur_fit, int8_t *best, uint32_t *best_fit);
 

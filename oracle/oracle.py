@@ -209,6 +209,50 @@ class Oracle:
             return list(ex.map(lambda c: self.run_chain(sched, c, n_steps, trace=trace), chains))
 
 
+def run_levels(orc: "Oracle", sched, n_chains: int, n_levels: int, group_size: int = 0, g0: int = 0,
+               states=None, threads: int = 1):
+    """PAPER.md Table 1 (:125-155), the level structure around the chain step, statement by statement:
+
+        while T > T_min:                                   # here: n_levels levels from step g0
+            for every thread: n_iterations chain steps     # steps_per_level x Oracle.run_chain (c-3)
+            d*_best = min_i d_best(i)                      # :150-151, per group; ties -> smallest chain
+            every x_best(i) = x*_best                      # :152-153
+            T = rho T                                      # level index from the step counter (reading 6)
+        (top of the next level: d_current = d_best; x_current = x_best, :129)
+
+    group_size = 0: one group of all chains (the paper); else groups of consecutive chains (its
+    future work, :321).  states = list of (cur, best, fit_cur, fit_best) per chain or None (fresh
+    chains, global ids chain_id_base + i).  Returns the list of states after the last level.
+    """
+    R = n_chains
+    group = R if group_size in (0, None) or group_size > R else group_size
+    base = getattr(sched, "chain_id_base", 0)
+    if states is None:
+        states = []
+        for c in range(R):
+            x, f = orc.init_chain(sched.seed, base + c)
+            states.append((x, x.copy(), f, f))
+    g = g0
+    assert g % sched.steps_per_level == 0, "levels start at level boundaries"
+    for _ in range(n_levels):
+        def advance(c):
+            out = orc.run_chain(sched, base + c, sched.steps_per_level, g0=g, state=states[c], trace=False)
+            return (out["cur"], out["best"], out["fit_cur"], out["fit_best"])
+        if threads > 1:
+            with ThreadPoolExecutor(threads) as ex:
+                states = list(ex.map(advance, range(R)))
+        else:
+            states = [advance(c) for c in range(R)]
+        g += sched.steps_per_level
+        for first in range(0, R, group):
+            members = range(first, min(R, first + group))
+            star = min(members, key=lambda c: (states[c][3], c))          # smallest d_best, then smallest chain
+            x_star, d_star = states[star][1], states[star][3]
+            for c in members:
+                states[c] = (x_star.copy(), x_star.copy(), d_star, d_star)
+    return states
+
+
 def simulate_fn(prob, params) -> np.ndarray:
     """The ``simulate`` callback problems.make_problem expects, served by the oracle."""
     return Oracle(prob).states_at_obs(params)

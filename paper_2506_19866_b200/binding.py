@@ -20,7 +20,7 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check")
+           "sa_select_kernel", "sa_jit_check", "sa_run_levels")
 SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
 
 if not os.path.exists(LIB_PATH):
@@ -58,6 +58,7 @@ FREE_FN = C.CFUNCTYPE(None, C.c_void_p)
 _lib.sa_last_error.restype = C.c_char_p
 _lib.sa_create.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.POINTER(_Schedule), C.POINTER(C.c_void_p)]
 _lib.sa_run.argtypes = [C.c_void_p, C.c_int64]
+_lib.sa_run_levels.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
 _lib.sa_best.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.sa_destroy.argtypes = [C.c_void_p]
 _lib.sa_destroy.restype = None
@@ -166,6 +167,10 @@ def sa_set_stream(h: int, stream: int) -> None:
 
 def sa_run(h: int, steps: int) -> None:
     _check(_lib.sa_run(h, steps), "sa_run")
+
+
+def sa_run_levels(h: int, n_levels: int, group_size: int = 0) -> None:
+    _check(_lib.sa_run_levels(h, n_levels, group_size), "sa_run_levels")
 
 
 def sa_best(h: int, n_params: int):

@@ -177,6 +177,7 @@ struct sa_handle {
   const tsa::StaticKernel* dk = nullptr;
   bool dk_tried = false;
   uint32_t* d_flags = nullptr;      // [R] hand-over flags of the balanced launch
+  unsigned long long* d_win = nullptr;   // [R] winners of the level synchronisation (sa_run_levels)
   int64_t last_slot_steps = 0;
   std::string dense_why;
   int family = SA_KERNEL_AUTO;
@@ -426,6 +427,28 @@ int sa_run(sa_handle* h, int64_t steps) {
     TSA_CUDA(tsa::launch_run(h->P, h->C, h->S, h->Tr, h->g, steps, h->threads, h->stream));
   ++h->launches;
   h->g += (uint64_t)steps;
+  return SA_OK;
+}
+
+int sa_run_levels(sa_handle* h, int64_t n_levels, int32_t group_size) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  if (n_levels < 0) return set_err(SA_EINVAL, "n_levels < 0");
+  if (group_size < 0) return set_err(SA_EINVAL, "group_size < 0");
+  if (h->g % (uint64_t)h->S.steps_per_level != 0)
+    return set_err(SA_EINVAL, "sa_run_levels must start at a level boundary (step counter % steps_per_level == 0)");
+  const int group = (group_size == 0 || group_size > h->C.R) ? h->C.R : group_size;
+  const int n_groups = (h->C.R + group - 1) / group;
+  if (!h->d_win) {
+    h->d_win = (unsigned long long*)h->pool.alloc((size_t)h->C.R * 8, h->stream);   // enough for any group size
+    if (!h->d_win) return set_err(SA_ENOMEM, "device allocation failed (level winners)");
+  }
+  (void)n_groups;
+  for (int64_t l = 0; l < n_levels; ++l) {
+    const int rc = sa_run(h, h->S.steps_per_level);
+    if (rc != SA_OK) return rc;
+    TSA_CUDA(tsa::launch_level_sync(h->P, h->C, group, h->d_win, h->stream));
+    h->launches += 2;
+  }
   return SA_OK;
 }
 

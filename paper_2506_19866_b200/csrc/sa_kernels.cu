@@ -575,6 +575,49 @@ cudaError_t launch_eval(const DevProblem& P, const int8_t* w, const int8_t* th, 
   return e != cudaSuccess ? e : cudaGetLastError();
 }
 
+// Level synchronisation of PAPER.md Table 1 (:150-155), on the device: per group of `group`
+// consecutive chains, the smallest d_best (ties: smallest chain) ...
+__global__ void group_argmin_kernel(const uint32_t* __restrict__ fit, int R, int group, unsigned long long* out) {
+  const int first = blockIdx.x * group, last = min(R, first + group);
+  unsigned long long best = ~0ull;
+  for (int c = first + (int)threadIdx.x; c < last; c += (int)blockDim.x)
+    best = min(best, ((unsigned long long)fit[c] << 32) | (unsigned)c);
+  __shared__ unsigned long long sm[32];
+  for (int o = 16; o > 0; o >>= 1) best = min(best, __shfl_down_sync(0xffffffffu, best, o));
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = best;
+  __syncthreads();
+  if (threadIdx.x < 32) {
+    best = threadIdx.x < (blockDim.x + 31) / 32 ? sm[threadIdx.x] : ~0ull;
+    for (int o = 16; o > 0; o >>= 1) best = min(best, __shfl_down_sync(0xffffffffu, best, o));
+    if (threadIdx.x == 0) out[blockIdx.x] = best;
+  }
+}
+
+// ... and its best vector becomes every member's best AND current vector ("use overall best
+// solution to re-initialize all threads"; x_current = x_best at the top of the next level).
+__global__ void level_broadcast_kernel(DevChains C, int EpadA, int NpadA, int group, const unsigned long long* __restrict__ win) {
+  const int c = blockIdx.x;
+  const unsigned long long w = win[c / group];
+  const int src = (int)(w & 0xFFFFFFFFull);
+  const uint32_t f = (uint32_t)(w >> 32);
+  const uint32_t* sw = (const uint32_t*)(C.best_w + (size_t)src * EpadA);
+  const uint32_t* sth = (const uint32_t*)(C.best_th + (size_t)src * NpadA);
+  uint32_t* cw = (uint32_t*)(C.cur_w + (size_t)c * EpadA);
+  uint32_t* cth = (uint32_t*)(C.cur_th + (size_t)c * NpadA);
+  uint32_t* bw = (uint32_t*)(C.best_w + (size_t)c * EpadA);
+  uint32_t* bth = (uint32_t*)(C.best_th + (size_t)c * NpadA);
+  for (int i = threadIdx.x; i < EpadA / 4; i += blockDim.x) { const uint32_t v = sw[i]; cw[i] = v; if (c != src) bw[i] = v; }
+  for (int i = threadIdx.x; i < NpadA / 4; i += blockDim.x) { const uint32_t v = sth[i]; cth[i] = v; if (c != src) bth[i] = v; }
+  if (threadIdx.x == 0) { C.fit_cur[c] = f; C.fit_best[c] = f; }
+}
+
+cudaError_t launch_level_sync(const DevProblem& P, const DevChains& C, int group, unsigned long long* win, cudaStream_t st) {
+  const int n_groups = (C.R + group - 1) / group;
+  group_argmin_kernel<<<n_groups, group >= 256 ? 256 : 32, 0, st>>>(C.fit_best, C.R, group, win);
+  level_broadcast_kernel<<<C.R, 128, 0, st>>>(C, P.EpadA, P.NpadA, group, win);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_argmin(const uint32_t* fit, int R, unsigned long long* out, cudaStream_t st) {
   argmin_kernel<<<1, 1024, 0, st>>>(fit, R, out);
   return cudaGetLastError();

@@ -18,6 +18,10 @@ cudaError_t launch_run_warp(const DevProblem& P, const DevChains& C, const DevSc
                             uint64_t g0, int64_t steps, int chains_per_cta, cudaStream_t st);
 cudaError_t launch_eval(const DevProblem& P, const int8_t* w, const int8_t* th, int64_t n, uint32_t* fit,
                         uint8_t* dump, int threads, cudaStream_t st);
+// PAPER.md Table 1 :150-155: per group of `group` consecutive chains, the member with the smallest
+// d_best (ties: smallest chain) gives its best vector to every member as best and current vector.
+// win = device scratch, one u64 per group.
+cudaError_t launch_level_sync(const DevProblem& P, const DevChains& C, int group, unsigned long long* win, cudaStream_t st);
 // out[0] = (fitness << 32) | chain of the best chain (smallest fitness, then smallest index)
 cudaError_t launch_argmin(const uint32_t* fit, int R, unsigned long long* out, cudaStream_t st);
 
