@@ -173,7 +173,7 @@ struct sa_handle {
   // dense (tensor-pipe) kernel (sa_dense_plan.h): host tables, device tables, the compiled kernel
   tsa::DensePlan dplan;
   const uint16_t *d_frag_slot = nullptr, *d_th_entry = nullptr;
-  const uint32_t *d_init_frag = nullptr, *d_obs_word = nullptr, *d_fix = nullptr, *d_dwloc = nullptr, *d_dthloc = nullptr;
+  const uint32_t *d_meta = nullptr, *d_init_frag = nullptr, *d_obs_word = nullptr, *d_fix = nullptr, *d_dwloc = nullptr, *d_dthloc = nullptr;
   const tsa::StaticKernel* dk = nullptr;
   bool dk_tried = false;
   uint32_t* d_flags = nullptr;      // [R] hand-over flags of the balanced launch
@@ -216,7 +216,7 @@ bool use_dense(sa_handle* h) {
 tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
   tsa_dense::Params q;
   std::memset(&q, 0, sizeof(q));
-  q.frag_slot = h->d_frag_slot; q.th_entry = h->d_th_entry; q.init_frag = h->d_init_frag;
+  q.frag_slot = h->d_frag_slot; q.meta = h->d_meta; q.th_entry = h->d_th_entry; q.init_frag = h->d_init_frag;
   q.obs_word = h->d_obs_word; q.fix = h->d_fix; q.wloc = h->d_dwloc; q.thloc = h->d_dthloc;
   std::memcpy(q.tha, h->P.tha, 16);
   std::memcpy(q.thb, h->P.thb, 16);
@@ -325,10 +325,12 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->plan.wloc, &h->d_wloc, st))) return rc;
     if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
   }
-  tsa::build_dense_plan(net, obs, h->plan, tsa::StaticTuning::from_env().dense_warps, &h->dplan);
+  tsa::build_dense_plan(net, obs, h->plan, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0,
+                        &h->dplan);
   if (h->dplan.ok) {
     if ((rc = h->pool.upload(h->dplan.frag_slot, &h->d_frag_slot, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.th_entry, &h->d_th_entry, st))) return rc;
+    if ((rc = h->pool.upload(h->dplan.meta, &h->d_meta, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.init_frag, &h->d_init_frag, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.obs_word, &h->d_obs_word, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.fix, &h->d_fix, st))) return rc;
@@ -622,7 +624,7 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
   if (rc != SA_OK) return set_err(rc, err);
   {
     tsa::DensePlan dp;
-    tsa::build_dense_plan(net, obs, pl, tsa::StaticTuning::from_env().dense_warps, &dp);
+    tsa::build_dense_plan(net, obs, pl, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0, &dp);
     if (dp.ok) {
       info[6] = 1;
       std::string cubin, clog;

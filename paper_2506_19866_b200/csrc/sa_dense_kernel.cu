@@ -37,6 +37,7 @@
 #define TSD_PH 1
 #define TSD_CPB 8
 #define TSD_REDERIVE 1
+#define TSD_SP 1
 #endif
 
 namespace tsa_dense {
@@ -49,7 +50,10 @@ constexpr int CPB = TSD_CPB;                    // chains per CTA (one-warp chai
 constexpr int WPW = NW / TW;                    // result words per condition a lane produces
 constexpr int MTW = 2 * WPW;                    // row tiles per warp (the last warp's may lie beyond MT)
 constexpr int PH = TSD_PH, WPP = WPW / PH;       // phases of a time step, result words per phase
-constexpr int NA = MTW * KS * 4;                // A-fragment registers per thread
+constexpr bool SP = TSD_SP != 0;                // 2:4-sparse A operand: mma.sp m16n8k64 (host guarantees <= 2 candidate edges per 4 columns)
+constexpr int KSP = KS / 2;                     // sparse steps of 64 columns
+constexpr int NA = SP ? MTW * KSP * 4 : MTW * KS * 4;   // A-fragment registers per thread
+constexpr int NM = SP ? MTW * KSP : 1;          // selector (metadata) registers per thread
 constexpr int STATE_BYTES = 8 * CS;             // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
 constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 2) * 4 + 15) / 16 * 16;   // bytes per chain
@@ -57,6 +61,7 @@ constexpr u64 kObsLo = TSD_OBSMASK_LO, kObsHi = TSD_OBSMASK_HI;
 constexpr u32 kOnes = 0x01010101u, kTwos = 0x02020202u;
 constexpr bool kByteMism = NOBS * 2 * NW <= 255;   // mismatch counters stay in byte lanes
 static_assert(KS == 1 || KS == 2 || KS == 4, "KS must be 1, 2 or 4");
+static_assert(!SP || KS % 2 == 0, "the sparse layout needs whole 64-column steps");
 static_assert(2 * KS >= MT && MT >= 1, "row <-> column numbering needs MT <= 2*KS");
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
 static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
@@ -90,6 +95,13 @@ __device__ __forceinline__ void imma(int (&c)[4], const u32* a, u32 b0, u32 b1) 
   asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// D (16 x 8, s32) += A (16 x 64, s8, 2:4 sparse: 16 x 32 stored + selectors e) * B (64 x 8, s8, col)
+__device__ __forceinline__ void imma_sp(int (&c)[4], const u32* a, u32 b0, u32 b1, u32 b2, u32 b3, u32 e) {
+  asm volatile("mma.sp::ordered_metadata.sync.aligned.m16n8k64.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9,%10,%11}, {%0,%1,%2,%3}, %12, 0x0;"
+               : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "r"(b2), "r"(b3), "r"(e));
 }
 
 __device__ __forceinline__ void team_sync() {
@@ -133,6 +145,7 @@ __device__ __forceinline__ void xor_reg(u32 (&a)[NA], int sel, u32 x) {
 // Everything a thread keeps in registers for the whole launch.
 struct Regs {
   u32 A[NA];        // the warp's rows of the weight matrix: A fragments of its tile (mi, s) at [(mi*KS + s)*4 .. +3]
+  u32 M[NM];        // sparse layout: selector words of the warp's tiles (the same for every chain)
   u32 TA[WPW];      // per byte (one row of this thread group): 0x80 - t_lo, padding rows 0
   u32 TD[WPW];      // minus, per byte: t_hi - t_lo + 1, padding rows 0
   u32 fix[NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows)
@@ -151,11 +164,21 @@ struct Phases {
     if (CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
 #pragma unroll
     for (int m = 0; m < 2 * WPP; ++m) { acc[m][0] = 0; acc[m][1] = 0; acc[m][2] = 0; acc[m][3] = 0; }
+    if (SP) {
 #pragma unroll
-    for (int s = 0; s < KS; ++s)
+      for (int s = 0; s < KSP; ++s)
 #pragma unroll
-      for (int mi = 0; mi < 2 * WPP; ++mi)
-        if (TW * MTW <= MT || 2 * W0 + mi < n_tiles) imma(acc[mi], &r.A[((2 * W0 + mi) * KS + s) * 4], b[2 * s], b[2 * s + 1]);
+        for (int mi = 0; mi < 2 * WPP; ++mi)
+          if (TW * MTW <= MT || 2 * W0 + mi < n_tiles)
+            imma_sp(acc[mi], &r.A[((2 * W0 + mi) * KSP + s) * 4], b[4 * s], b[4 * s + 1], b[4 * s + 2], b[4 * s + 3],
+                    r.M[SP ? (2 * W0 + mi) * KSP + s : 0]);
+    } else {
+#pragma unroll
+      for (int s = 0; s < KS; ++s)
+#pragma unroll
+        for (int mi = 0; mi < 2 * WPP; ++mi)
+          if (TW * MTW <= MT || 2 * W0 + mi < n_tiles) imma(acc[mi], &r.A[((2 * W0 + mi) * KS + s) * 4], b[2 * s], b[2 * s + 1]);
+    }
     if (CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
     u32 ns[2][WPP];
 #pragma unroll
@@ -366,6 +389,8 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     const u32 b3 = o3 == 0xFFFFu ? 0u : (u32)(unsigned char)cw[o3];
     r.A[i] = b0 | (b1 << 8) | (b2 << 16) | (b3 << 24);
   }
+#pragma unroll
+  for (int i = 0; i < NM; ++i) r.M[i] = SP ? __ldg(p.meta + (ww * NM + i) * 32 + lane) : 0u;
 #pragma unroll
   for (int w = 0; w < WPW; ++w) {
     u32 ta = 0u, td = 0u;

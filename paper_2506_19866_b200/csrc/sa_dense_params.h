@@ -19,6 +19,7 @@ typedef signed char i8;
 struct Params {
   // problem tables (one per problem, shared by all chains)
   const u16* frag_slot;   // [MT*KS*4][32][4] canonical weight-row offset feeding each A-fragment byte, 0xFFFF = structural zero
+  const u32* meta;        // [tiles][32] sparse layout: selector word of each A tile, per lane
   const u16* th_entry;    // [8][NW][4]        canonical threshold-row offset of the node in (group g, word w, byte j), 0xFFFF = padding row
   const u32* init_frag;   // [32][2*KS]        B fragments of the t = 0 states, per lane
   const u32* obs_word;    // [NOBS][32][2*NW]  observed values in the layout of a lane's result words (3 = not scored)

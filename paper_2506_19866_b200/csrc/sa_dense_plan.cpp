@@ -54,9 +54,54 @@ void pick_strides(int KS, int W, int* CS, int* TS, int* wf) {
   *wf = best;
 }
 
+// Node -> row assignment for the 2:4-sparse layout.  Four consecutive matrix columns are the rows
+// {32w + g + 8j : j = 0..3} (see col_of_row below); a row of W may hold at most two candidate
+// edges in any such group.  Local search over swaps and moves (deterministic), starting from the
+// identity; returns false if some violation is left.
+bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::vector<std::vector<int>>& out_dst,
+                      int n_rows, std::vector<int>* row_of_node) {
+  const int N = (int)in_src.size();
+  std::vector<int>& row = *row_of_node;
+  std::vector<int> node_at(n_rows, -1);
+  for (int i = 0; i < N; ++i) node_at[row[i]] = i;
+  auto group_of = [&](int r) { return (r / 32) * 8 + r % 8; };
+  auto row_cost = [&](int i) {
+    int cnt[64] = {0}, c = 0;
+    for (int s : in_src[i]) if (++cnt[group_of(row[s])] > 2) ++c;
+    return c;
+  };
+  long cost = 0;
+  for (int i = 0; i < N; ++i) cost += row_cost(i);
+  uint64_t st = 0x9E3779B97F4A7C15ull;
+  auto rnd = [&](int n) {
+    st ^= st >> 12; st ^= st << 25; st ^= st >> 27;
+    return (int)((((st * 0x2545F4914F6CDD1Dull) >> 32) * (uint64_t)n) >> 32);
+  };
+  for (long it = 0; cost > 0 && it < 400000; ++it) {
+    const int a = rnd(N), r2 = rnd(n_rows), b = node_at[r2];
+    if (r2 == row[a] || (b >= 0 && group_of(row[b]) == group_of(row[a]))) continue;
+    long before = 0, after = 0;
+    for (int i : out_dst[a]) before += row_cost(i);
+    if (b >= 0) for (int i : out_dst[b]) before += row_cost(i);
+    const int ra = row[a];
+    row[a] = r2; if (b >= 0) row[b] = ra;
+    for (int i : out_dst[a]) after += row_cost(i);
+    if (b >= 0) for (int i : out_dst[b]) after += row_cost(i);
+    if (after <= before) {                 // rows fed by both a and b are counted twice on both sides
+      node_at[r2] = a; node_at[ra] = b;
+      cost = 0;
+      if (after != before) for (int i = 0; i < N; ++i) cost += row_cost(i); else for (int i = 0; i < N; ++i) cost += row_cost(i);
+    } else {
+      row[a] = ra; if (b >= 0) row[b] = r2;
+    }
+  }
+  return cost == 0;
+}
+
 }  // namespace
 
-void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& pl, int team_warps, DensePlan* dp) {
+void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& pl, int team_warps, bool want_sparse,
+                      DensePlan* dp) {
   *dp = DensePlan();
   const int N = pl.N, E = pl.E, K = pl.K, NO = pl.n_obs;
   if (N > 128) { dp->why = "more than 128 nodes"; return; }
@@ -75,59 +120,104 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
 
   // Row r = 16m + 8h + g is produced by thread group g as byte j of its word w, q = 2m + h = 4w + j.
   // That byte is stored at chunk t' = g % 4, word pos = (g / 4) * NW + w, which B-fragment thread t'
-  // reads as column k = 32*(pos/2) + 16*(pos%2) + 4t' + j.  Node i sits at row i.
+  // reads as column k = 16*pos + 4t' + j.
   auto col_of_row = [&](int r) {
     const int m = r / 16, h = (r % 16) / 8, g = r % 8, q = 2 * m + h, w = q / 4, j = q % 4;
     const int pos = (g / 4) * NW + w;
-    return 32 * (pos / 2) + 16 * (pos % 2) + 4 * (g % 4) + j;
+    return 16 * pos + 4 * (g % 4) + j;
   };
+  // node -> row: the identity, or (sparse layout) a permutation that puts at most two of any node's
+  // sources into the same group of four columns
+  std::vector<int> row_of_node(N);
+  for (int i = 0; i < N; ++i) row_of_node[i] = i;
+  if (want_sparse && KS % 2 == 0) {
+    std::vector<std::vector<int>> in_src(N), out_dst(N);
+    for (int e = 0; e < E; ++e) { in_src[net->edge_dst[e]].push_back(net->edge_src[e]); out_dst[net->edge_src[e]].push_back(net->edge_dst[e]); }
+    std::vector<int> trial = row_of_node;
+    if (assign_rows_2of4(in_src, out_dst, 16 * MT, &trial)) { row_of_node = trial; dp->sparse = true; }
+  }
+  const int KSP = KS / 2;                            // sparse steps of 64 columns
+  std::vector<int> node_of_row(32 * KS, -1), node_of_col(32 * KS, -1);
+  for (int i = 0; i < N; ++i) { node_of_row[row_of_node[i]] = i; node_of_col[col_of_row(row_of_node[i])] = i; }
   auto state_offset = [&](int cond, int node) {     // byte of (cond, node) in the exchange buffer
-    const int k = col_of_row(node), s = k / 32, hf = (k % 32) / 16, tq = (k % 16) / 4, j = k % 4;
-    return cond * CS + tq * TS + (2 * s + hf) * 4 + j;
+    const int k = col_of_row(row_of_node[node]), pos = k / 16, tq = (k % 16) / 4, j = k % 4;
+    return cond * CS + tq * TS + pos * 4 + j;
   };
-  std::vector<int> node_of_col(32 * KS, -1);
-  for (int i = 0; i < N; ++i) node_of_col[col_of_row(i)] = i;
-
-  // A fragments: register (m, s, a) of lane (g, t) holds row 16m + g + 8(a&1), columns 32s + 16(a>>1) + 4t + 0..3;
-  // row tile m belongs to warp m / MTW as its tile m % MTW
   std::map<std::pair<int, int>, int> edge_at;       // (dst, src) -> edge
   for (int e = 0; e < E; ++e) edge_at[{net->edge_dst[e], net->edge_src[e]}] = e;
-  const int NA = 2 * NW * KS * 4;
-  dp->frag_slot.assign((size_t)NA * 32 * 4, 0xFFFFu);
+  auto edge_of = [&](int row, int col) {            // candidate edge at matrix position (row, col) or -1
+    if (node_of_row[row] < 0 || node_of_col[col] < 0) return -1;
+    auto it = edge_at.find({node_of_row[row], node_of_col[col]});
+    return it == edge_at.end() ? -1 : it->second;
+  };
   dp->wloc.assign(E, 0u);
-  for (int m = 0; m < 2 * NW; ++m)
-    for (int s = 0; s < KS; ++s)
-      for (int a = 0; a < 4; ++a)
-        for (int lane = 0; lane < 32; ++lane)
-          for (int b = 0; b < 4; ++b) {
-            const int g = lane / 4, t = lane % 4, reg = (m * KS + s) * 4 + a;
-            const int row = 16 * m + g + 8 * (a & 1), col = 32 * s + 16 * (a >> 1) + 4 * t + b;
-            if (row >= N || node_of_col[col] < 0) continue;
-            auto it = edge_at.find({row, node_of_col[col]});
-            if (it == edge_at.end()) continue;
-            const int e = it->second, slot = pl.slot_of_param[e];
-            dp->frag_slot[((size_t)reg * 32 + lane) * 4 + b] = (uint16_t)slot;
-            const int ww = m / MTW, wreg = ((m % MTW) * KS + s) * 4 + a;
-            dp->wloc[e] = (uint32_t)wreg | ((uint32_t)b << 7) | ((uint32_t)lane << 9) | ((uint32_t)ww << 14) | ((uint32_t)slot << 16);
-          }
-  // thresholds: byte j of word w of thread group g <-> row
+  auto place = [&](int e, int m, int wreg, int lane, int b, int global_reg) {
+    const int slot = pl.slot_of_param[e];
+    dp->frag_slot[((size_t)global_reg * 32 + lane) * 4 + b] = (uint16_t)slot;
+    dp->wloc[e] = (uint32_t)wreg | ((uint32_t)b << 7) | ((uint32_t)lane << 9) | ((uint32_t)(m / MTW) << 14) | ((uint32_t)slot << 16);
+  };
+  const int tiles = 2 * NW;                          // row tiles padded to whole warps
+  if (!dp->sparse) {
+    // dense A fragments: register (m, s, a) of lane (g, t) holds row 16m + g + 8(a&1), columns 32s + 16(a>>1) + 4t + 0..3;
+    // row tile m belongs to warp m / MTW as its tile m % MTW
+    dp->frag_slot.assign((size_t)tiles * KS * 4 * 32 * 4, 0xFFFFu);
+    for (int m = 0; m < tiles; ++m)
+      for (int s = 0; s < KS; ++s)
+        for (int a = 0; a < 4; ++a)
+          for (int lane = 0; lane < 32; ++lane)
+            for (int b = 0; b < 4; ++b) {
+              const int g = lane / 4, t = lane % 4;
+              const int e = edge_of(16 * m + g + 8 * (a & 1), 32 * s + 16 * (a >> 1) + 4 * t + b);
+              if (e >= 0) place(e, m, ((m % MTW) * KS + s) * 4 + a, lane, b, (m * KS + s) * 4 + a);
+            }
+    dp->meta.assign(32, 0u);
+  } else {
+    // 2:4-sparse A (mma.sp m16n8k64, layout measured on sm_100a): tile (m, sp) covers columns 64sp .. 64sp+63
+    // in 16 groups of four.  Per row and group two slots are stored: byte 2*(G%2) + slot of register
+    // a = 2*(G/8) + half in lane 4g + (G%8)/2, and a 4-bit selector (position of slot 0, position of
+    // slot 1 << 2, ascending) in nibble G%8 of the metadata word of lane 4g + 2*(G/8) + half.
+    dp->frag_slot.assign((size_t)tiles * KSP * 4 * 32 * 4, 0xFFFFu);
+    dp->meta.assign((size_t)tiles * KSP * 32, 0u);
+    for (int m = 0; m < tiles; ++m)
+      for (int sp = 0; sp < KSP; ++sp)
+        for (int g = 0; g < 8; ++g)
+          for (int half = 0; half < 2; ++half)
+            for (int G = 0; G < 16; ++G) {
+              int pos[4], edges[4], n = 0;
+              for (int pp = 0; pp < 4; ++pp) {
+                const int e = edge_of(16 * m + g + 8 * half, 64 * sp + 4 * G + pp);
+                if (e >= 0) { pos[n] = pp; edges[n] = e; ++n; }
+              }
+              if (n > 2) { dp->why = "internal error: more than two candidate edges in a 2:4 group"; return; }
+              int idx0 = 0, idx1 = 1, e0 = -1, e1 = -1;
+              if (n == 2) { idx0 = pos[0]; idx1 = pos[1]; e0 = edges[0]; e1 = edges[1]; }
+              else if (n == 1 && pos[0] < 3) { idx0 = pos[0]; idx1 = pos[0] + 1; e0 = edges[0]; }
+              else if (n == 1) { idx0 = 2; idx1 = 3; e1 = edges[0]; }
+              const int tile = m * KSP + sp, a = 2 * (G / 8) + half, lane = 4 * g + (G % 8) / 2;
+              dp->meta[(size_t)tile * 32 + 4 * g + 2 * (G / 8) + half] |= (uint32_t)(idx0 | (idx1 << 2)) << (4 * (G % 8));
+              const int wreg = ((m % MTW) * KSP + sp) * 4 + a;
+              if (e0 >= 0) place(e0, m, wreg, lane, 2 * (G % 2), tile * 4 + a);
+              if (e1 >= 0) place(e1, m, wreg, lane, 2 * (G % 2) + 1, tile * 4 + a);
+            }
+  }
+  // thresholds: byte j of word w of thread group g <-> row 32w + 8j + g
   dp->th_entry.assign((size_t)8 * NW * 4, 0xFFFFu);
   dp->thloc.assign(N, 0u);
   for (int g = 0; g < 8; ++g)
     for (int w = 0; w < NW; ++w)
       for (int j = 0; j < 4; ++j) {
-        const int q = 4 * w + j, row = 16 * (q / 2) + 8 * (q % 2) + g;
-        if (row >= N || q / 2 >= MT) continue;
-        const int entry = pl.entry_of_node[row];
+        const int row = 32 * w + 8 * j + g;
+        if (row >= 16 * MT || node_of_row[row] < 0) continue;
+        const int node = node_of_row[row], entry = pl.entry_of_node[node];
         dp->th_entry[((size_t)g * NW + w) * 4 + j] = (uint16_t)entry;
-        dp->thloc[row] = (uint32_t)g | ((uint32_t)w << 3) | ((uint32_t)j << 5) | ((uint32_t)entry << 16);
+        dp->thloc[node] = (uint32_t)g | ((uint32_t)w << 3) | ((uint32_t)j << 5) | ((uint32_t)entry << 16);
       }
-  // t = 0 states as B fragments: lane (g', t') word 2s + hf = columns 32s + 16hf + 4t' + 0..3 of condition g'
+  // t = 0 states as B fragments: lane (g', t') word pos = columns 16 pos + 4t' + 0..3 of condition g'
   dp->init_frag.assign((size_t)32 * 2 * KS, 0u);
   for (int lane = 0; lane < 32; ++lane)
     for (int x = 0; x < 2 * KS; ++x)
       for (int j = 0; j < 4; ++j) {
-        const int cond = lane / 4, col = 32 * (x / 2) + 16 * (x % 2) + 4 * (lane % 4) + j;
+        const int cond = lane / 4, col = 16 * x + 4 * (lane % 4) + j;
         if (cond >= K || node_of_col[col] < 0) continue;
         dp->init_frag[(size_t)lane * 2 * KS + x] |= (uint32_t)obs->init_state[(size_t)cond * N + node_of_col[col]] << (8 * j);
       }
@@ -137,7 +227,7 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   for (int k = 0; k < K; ++k)
     for (int i = 0; i < N; ++i)
       if (obs->clamp[(size_t)k * N + i]) {
-        const int q = 2 * (i / 16) + (i % 16) / 8, ww = (q / 4) / WPW;
+        const int ww = (row_of_node[i] / 32) / WPW;
         fixes[ww].push_back((uint32_t)state_offset(k, i) | ((uint32_t)obs->init_state[(size_t)k * N + i] << 16) | 0x80000000u);
       }
   dp->n_fix_rounds = 1;
@@ -154,12 +244,13 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
         for (int c = 0; c < 2; ++c)
           for (int w = 0; w < NW; ++w)
             for (int j = 0; j < 4; ++j) {
-              const int g = lane / 4, t = lane % 4, cond = 2 * t + c, q = 4 * w + j, row = 16 * (q / 2) + 8 * (q % 2) + g;
-              if (row >= N || q / 2 >= MT || cond >= K) continue;
-              const uint8_t o = obs->obs[((size_t)cond * NO + oj) * N + row];
+              const int g = lane / 4, t = lane % 4, cond = 2 * t + c, row = 32 * w + 8 * j + g;
+              if (row >= 16 * MT || node_of_row[row] < 0 || cond >= K) continue;
+              const int node = node_of_row[row];
+              const uint8_t o = obs->obs[((size_t)cond * NO + oj) * N + node];
               if (o == SA_UNOBSERVED) continue;
-              if (obs->clamp[(size_t)cond * N + row]) {
-                if (o != obs->init_state[(size_t)cond * N + row]) ++clamped_mis;
+              if (obs->clamp[(size_t)cond * N + node]) {
+                if (o != obs->init_state[(size_t)cond * N + node]) ++clamped_mis;
                 continue;
               }
               uint32_t& word = dp->obs_word[((size_t)oj * 32 + lane) * 2 * NW + c * NW + w];
@@ -168,6 +259,12 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
             }
   }
   dp->fit_const = (int)(clamped_mis - always);
+  {                                                  // self-check: every edge sits in exactly one fragment byte
+    std::vector<int> seen(pl.EpadA, 0);
+    for (uint16_t s : dp->frag_slot) if (s != 0xFFFFu) ++seen[s];
+    for (int e = 0; e < E; ++e)
+      if (seen[pl.slot_of_param[e]] != 1) { dp->why = "internal error: edge not placed exactly once"; return; }
+  }
   dp->ok = true;
 }
 

@@ -15,12 +15,14 @@ struct DensePlan {
   bool ok = false;
   std::string why;          // reason when !ok
   int MT = 0, KS = 0;       // 16-row tiles, 32-column steps (KS = result words per condition and thread group)
+  bool sparse = false;      // 2:4-sparse A operand (mma.sp m16n8k64): nodes permuted so that every row has <= 2 candidates per 4 columns
   int W = 1;                // warps per chain; warp ww owns result words ww*KS/W .. and their row tiles
   int CS = 0, TS = 0;       // byte strides of the exchange buffer: per condition, per B-fragment thread chunk
   int exchange_wavefronts = 0;   // shared-memory wavefronts of one exchange (2 stores + 2 loads)
   int n_fix_rounds = 1;
   int fit_const = 0;
-  std::vector<uint16_t> frag_slot;   // [2*KS*KS*4][32][4] (row tiles padded to 2*KS)
+  std::vector<uint16_t> frag_slot;   // [2*KS * (sparse ? KS/2 : KS) * 4][32][4] (row tiles padded to 2*KS)
+  std::vector<uint32_t> meta;        // sparse: [2*KS * KS/2][32] selector words, one per tile and lane
   std::vector<uint16_t> th_entry;    // [8][KS][4]
   std::vector<uint32_t> init_frag;   // [32][2*KS]
   std::vector<uint32_t> obs_word;    // [n_obs][32][2*KS]
@@ -34,6 +36,7 @@ struct DensePlan {
 
 // Applies when N <= 128 and K <= 8.  team_warps = warps per chain (1, 2 or 4; reduced until it
 // divides KS).  Always returns; check dp->ok / dp->why.
-void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& plan, int team_warps, DensePlan* dp);
+void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& plan, int team_warps, bool want_sparse,
+                      DensePlan* dp);
 
 }  // namespace tsa
