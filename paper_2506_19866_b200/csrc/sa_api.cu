@@ -206,7 +206,7 @@ bool use_dense(sa_handle* h) {
     if (!std::getenv("TSA_DENSE_BLOCKS")) {
       // fewer chains than slots: do not squeeze the registers for an occupancy the grid cannot reach
       const int per_sm = (int)((h->C.R + h->sm_count - 1) / std::max(h->sm_count, 1));
-      tune.dense_blocks = std::max(1, std::min(tune.dense_blocks, per_sm));
+      tune.dense_blocks = std::max(1, std::min(h->dplan.sparse ? 16 : 12, per_sm));
     }
     h->dk = tsa::dense_kernel_get(h->plan, h->dplan, tune, &h->dense_why);
   }

@@ -18,7 +18,8 @@ struct StaticTuning {
   int max_regs = 128;     // register budget per thread -> __launch_bounds__ min blocks
   int batch = 8;          // state gathers issued back to back before their IMADs
   int t_unroll = 1;       // unroll factor of the time loop
-  int dense_blocks = 12;  // dense kernel: resident chains (CTAs) per SM the register allocation aims at (12 -> 168 registers)
+  int dense_blocks = 0;   // dense kernel: resident chains (CTAs) per SM the register allocation aims at; 0 = 16 (128
+                          // registers) with the sparse A operand, 12 (168 registers) with the dense one
   int dense_phases = 1;   // dense kernel: phases of a time step (accumulator tiles live at a time = row tiles / phases)
   int dense_cpb = 1;      // dense kernel: one-warp chains per CTA (1, 4, 8 or 12); > 1 turns the tensor-pipe token ring on
   int dense_sparse = 1;   // dense kernel: use the 2:4-sparse A operand (mma.sp) when the network allows it

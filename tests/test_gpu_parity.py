@@ -251,6 +251,8 @@ FAMILY_CASES = [
     ("mtb", "DENSE", {"TSA_DENSE_BLOCKS": "8"}), ("mtb", "DENSE", {"TSA_DENSE_PH": "2"}),
     ("mtb", "DENSE", {"TSA_DENSE_CPB": "8"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "12"}),
     ("hpg", "DENSE", {"TSA_DENSE_CPB": "4"}),
+    ("mtb", "DENSE", {"TSA_DENSE_SP": "0"}), ("mtb", "DENSE", {"TSA_DENSE_SP": "0", "TSA_DENSE_W": "2"}),
+    ("mtb", "DENSE", {"TSA_DENSE_SP": "0", "TSA_DENSE_CPB": "8"}),
 ]
 
 
