@@ -144,6 +144,7 @@ def run_ours(args) -> dict:
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         info = None
         best = None
+        dense = None
         for it in range(warmup + steps):
             h = B.sa_create(prob, sched)
             flush.fill_(it & 0xFF)
@@ -157,12 +158,13 @@ def run_ours(args) -> dict:
             if it == warmup + steps - 1:
                 barrier()
                 info = B.sa_get_info(h)
+                dense = B.sa_get_dense_info(h)
                 best = B.sa_best(h, prob.n_params)
             B.sa_destroy(h)
         ms = [a.elapsed_time(b) for a, b in ev]
         kernel_ms = sum(ms)
         total_ms = max_over_ranks(kernel_ms, dist)
-        res = {"prob": prob, "sched": sched, "ms": ms, "total_ms": total_ms, "info": info, "best": best,
+        res = {"prob": prob, "sched": sched, "ms": ms, "total_ms": total_ms, "info": info, "best": best, "dense": dense,
                "chain_steps": chains * sa_steps * steps * world}
         if want_e2e:
             # end to end through the public API: host buffers in, best vector out, every step
@@ -249,11 +251,14 @@ def run_ours(args) -> dict:
         if main["info"]["variant"] == 5:
             # second ceiling of the dense kernel: MT*KS IMMA.16832.S8 per time step against the measured
             # 0.5 IMMA per clock per SM of the legacy tensor path on B200
-            mt = (prob.n_nodes + 15) // 16
-            ks = {1: 1, 2: 2, 3: 4, 4: 4}[(mt + 1) // 2]
-            immas = prob.n_steps * mt * ks * chains * sa_steps / kernel_s
-            out["roofline"]["tensor_pipe"] = {"imma_per_chain_step": prob.n_steps * mt * ks, "achieved_imma_per_s": immas,
-                                              "peak_imma_per_s": 0.5 * sms * sm_max_hz, "frac": immas / (0.5 * sms * sm_max_hz)}
+            di = main["dense"]
+            per_step = prob.n_steps * di["row_tiles"] * (di["col_steps"] // 2 if di["sparse"] else di["col_steps"])
+            rate = 0.443 if di["sparse"] else 0.5     # measured: IMMA.SP.16864 / IMMA.16832 per clock per SM
+            immas = per_step * chains * sa_steps / kernel_s
+            out["roofline"]["tensor_pipe"] = {"imma_per_chain_step": per_step, "sparse_2of4": bool(di["sparse"]),
+                                              "achieved_imma_per_s": immas, "peak_imma_per_s": rate * sms * sm_max_hz,
+                                              "frac": immas / (rate * sms * sm_max_hz)}
+            out["config"]["dense"] = di
         if world == 1 and not args.no_extra:
             try:
                 pk = B.sa_int32_peak()

@@ -138,6 +138,13 @@ int sa_geometric_table(double t0, double t_end, int32_t n_levels, int32_t dmax, 
  * The variant is decided at the first sa_run; before it, info[0] reports the generic choice. */
 int sa_get_info(sa_handle *h, int64_t info[16]);
 
+/* Shape of the dense kernel for this handle: info[0] = 1 if it applies (else all zero), [1] = 16-row
+ * tiles MT, [2] = 32-column steps KS, [3] = 1 if the 2:4-sparse A operand is used (mma.sp m16n8k64:
+ * MT * KS/2 IMMAs per time step instead of MT * KS), [4] = warps per chain, [5] = resident CTAs per
+ * SM of the loaded kernel (0 before the first sa_run), [6] = chain-steps per slot of the last sa_run
+ * if it used balanced slots (else 0), [7] = shared-memory wavefronts of one state exchange. */
+int sa_get_dense_info(sa_handle *h, int64_t info[8]);
+
 /* Kernel family of sa_run.  AUTO (default): the dense kernel — the node update as an int8 product
  * on the tensor pipe with the chain's weight matrix in mma.sync fragments — when the
  * network has at most 128 nodes and 8 conditions; else the statically scheduled gather kernel —

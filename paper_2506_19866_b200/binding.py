@@ -20,7 +20,7 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check", "sa_run_levels")
+           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info")
 SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
 
 if not os.path.exists(LIB_PATH):
@@ -70,6 +70,7 @@ _lib.sa_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64]
 _lib.sa_get_trace.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_geometric_table.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_void_p]
 _lib.sa_get_info.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sa_get_dense_info.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_plan_info.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c_void_p]
 _lib.sa_set_stream.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_set_allocator.argtypes = [C.c_void_p, C.c_void_p]
@@ -232,6 +233,13 @@ def sa_get_info(h: int) -> dict:
     keys = ("variant", "threads_per_cta", "chains_per_cta", "smem_bytes", "grid", "edge_slots", "sm_count", "launches",
             "passes", "edge_iterations", "rows", "split_nodes", "state_words_per_node", "state_entries",
             "static_regs", "team_warps")
+    return dict(zip(keys, (int(v) for v in info)))
+
+
+def sa_get_dense_info(h: int) -> dict:
+    info = np.zeros(8, dtype=np.int64)
+    _check(_lib.sa_get_dense_info(h, info.ctypes.data), "sa_get_dense_info")
+    keys = ("applies", "row_tiles", "col_steps", "sparse", "team_warps", "ctas_per_sm", "slot_steps", "exchange_wavefronts")
     return dict(zip(keys, (int(v) for v in info)))
 
 

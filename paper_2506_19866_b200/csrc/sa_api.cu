@@ -670,6 +670,21 @@ int sa_plan_info(const sa_network* net, const sa_observations* obs, int64_t info
   return SA_OK;
 }
 
+int sa_get_dense_info(sa_handle* h, int64_t info[8]) {
+  if (!h || !info) return set_err(SA_EINVAL, "null argument");
+  for (int i = 0; i < 8; ++i) info[i] = 0;
+  if (!h->dplan.ok) return SA_OK;
+  info[0] = 1;
+  info[1] = h->dplan.MT;
+  info[2] = h->dplan.KS;
+  info[3] = h->dplan.sparse ? 1 : 0;
+  info[4] = h->dplan.W;
+  info[5] = h->dk ? h->dk->blocks_per_sm : 0;
+  info[6] = h->last_slot_steps;
+  info[7] = h->dplan.exchange_wavefronts;
+  return SA_OK;
+}
+
 int sa_get_info(sa_handle* h, int64_t info[16]) {
   if (!h || !info) return set_err(SA_EINVAL, "null argument");
   for (int i = 0; i < 16; ++i) info[i] = 0;
