@@ -326,7 +326,7 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
   }
   tsa::build_dense_plan(net, obs, h->plan, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0,
-                        &h->dplan);
+                        tsa::StaticTuning::from_env().dense_swizzle != 0, &h->dplan);
   if (h->dplan.ok) {
     if ((rc = h->pool.upload(h->dplan.frag_slot, &h->d_frag_slot, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.th_entry, &h->d_th_entry, st))) return rc;
@@ -624,7 +624,8 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
   if (rc != SA_OK) return set_err(rc, err);
   {
     tsa::DensePlan dp;
-    tsa::build_dense_plan(net, obs, pl, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0, &dp);
+    tsa::build_dense_plan(net, obs, pl, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0,
+                          tsa::StaticTuning::from_env().dense_swizzle != 0, &dp);
     if (dp.ok) {
       info[6] = 1;
       std::string cubin, clog;

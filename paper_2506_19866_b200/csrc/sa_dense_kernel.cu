@@ -38,6 +38,7 @@
 #define TSD_CPB 8
 #define TSD_REDERIVE 1
 #define TSD_SP 1
+#define TSD_SWZ 1
 #endif
 
 namespace tsa_dense {
@@ -54,7 +55,8 @@ constexpr bool SP = TSD_SP != 0;                // 2:4-sparse A operand: mma.sp 
 constexpr int KSP = KS / 2;                     // sparse steps of 64 columns
 constexpr int NA = SP ? MTW * KSP * 4 : MTW * KS * 4;   // A-fragment registers per thread
 constexpr int NM = SP ? MTW * KSP : 1;          // selector (metadata) registers per thread
-constexpr int STATE_BYTES = 8 * CS;             // one exchange buffer: 8 condition rows
+constexpr bool SWZ = TSD_SWZ != 0;              // swizzled exchange buffer (KS = 4, one warp per chain): conflict-free stores AND loads
+constexpr int STATE_BYTES = SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
 constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 2) * 4 + 15) / 16 * 16;   // bytes per chain
 constexpr u64 kObsLo = TSD_OBSMASK_LO, kObsHi = TSD_OBSMASK_HI;
@@ -62,6 +64,7 @@ constexpr u32 kOnes = 0x01010101u, kTwos = 0x02020202u;
 constexpr bool kByteMism = NOBS * 2 * NW <= 255;   // mismatch counters stay in byte lanes
 static_assert(KS == 1 || KS == 2 || KS == 4, "KS must be 1, 2 or 4");
 static_assert(!SP || KS % 2 == 0, "the sparse layout needs whole 64-column steps");
+static_assert(!SWZ || (KS == 4 && TSD_W == 1), "the swizzled exchange buffer is for 16-byte units of one warp");
 static_assert(2 * KS >= MT && MT >= 1, "row <-> column numbering needs MT <= 2*KS");
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
 static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
@@ -158,7 +161,7 @@ struct Regs {
 template <int P>
 struct Phases {
   static __device__ __forceinline__ void run(const Regs& r, const u32 (&b)[2 * KS], int n_tiles, bool is_obs, const u32* ow,
-                                             u32& cnt, bool store, u32 st, int ring_me, int ring_next) {
+                                             u32& cnt, bool store, u32 st, u32 st1, int ring_me, int ring_next) {
     constexpr int W0 = P * WPP;
     int acc[2 * WPP][4];
     if (CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
@@ -202,14 +205,14 @@ struct Phases {
     }
     if (store) {
       sts_vec(st + W0 * 4, ns[0]);
-      sts_vec(st + W0 * 4 + CS, ns[1]);
+      sts_vec(st1 + W0 * 4, ns[1]);
     }
-    Phases<P + 1>::run(r, b, n_tiles, is_obs, ow, cnt, store, st, ring_me, ring_next);
+    Phases<P + 1>::run(r, b, n_tiles, is_obs, ow, cnt, store, st, st1, ring_me, ring_next);
   }
 };
 template <>
 struct Phases<PH> {
-  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], int, bool, const u32*, u32&, bool, u32, int, int) {}
+  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], int, bool, const u32*, u32&, bool, u32, u32, int, int) {}
 };
 
 // a3 + a4 for the parameters now in registers: returns the team's mismatch count.
@@ -217,9 +220,26 @@ struct Phases<PH> {
 __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf, volatile u32* red, int parity, int lane, int ww,
                                         int ring_me, int ring_next) {
   const int g = lane >> 2, t4 = lane & 3;
-  u32 st_addr = sbuf + (u32)((2 * t4) * CS + (g & 3) * TS + ((g >> 2) * NW + ww * WPW) * 4);
-  u32 ld_addr = sbuf + (u32)(g * CS + t4 * TS);
+  // Exchange buffer.  Plain layout: condition rows of CS bytes, thread chunks of TS bytes (strides from
+  // the host's conflict search).  Swizzled layout (16-byte units, unit (c, t', half) = the words
+  // 4*half .. 4*half+3 of chunk t' of condition c): 128-byte row 4*half + c/2, 16-byte column
+  // 4*(t'&1) + (c/2 + 2*(t'/2) + (c&1)) mod 4 -- a Latin square, so that the eight lanes of a quarter
+  // warp hit eight different columns both when they store (c/2 and t'&1 vary) and when they load
+  // (c&1, t'/2 and t'&1 vary).
+  u32 st_addr, st_delta, ld_addr;
+  if (SWZ) {
+    const int tq = g & 3, half = g >> 2;
+    const int q0 = 4 * (tq & 1) + ((t4 + 2 * (tq >> 1)) & 3), q1 = 4 * (tq & 1) + ((t4 + 2 * (tq >> 1) + 1) & 3);
+    st_addr = sbuf + (u32)((4 * half + t4) * 128 + q0 * 16);
+    st_delta = (u32)((q1 - q0) * 16);
+    ld_addr = sbuf + (u32)((g >> 1) * 128 + (4 * (t4 & 1) + (((g >> 1) + 2 * (t4 >> 1) + (g & 1)) & 3)) * 16);
+  } else {
+    st_addr = sbuf + (u32)((2 * t4) * CS + (g & 3) * TS + ((g >> 2) * NW + ww * WPW) * 4);
+    st_delta = (u32)CS;
+    ld_addr = sbuf + (u32)(g * CS + t4 * TS);
+  }
   asm volatile("" : "+r"(st_addr), "+r"(ld_addr));      // keep them in registers (no S2R in the loop)
+  if (SWZ) asm volatile("" : "+r"(st_delta));
   const int n_tiles = MT - ww * MTW;                      // row tiles of this warp that exist (warp-uniform)
   u32 b[2 * KS];
   {
@@ -236,7 +256,7 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
     const u32 boff = NBUF == 2 ? (u32)(t & 1) * STATE_BYTES : 0u;
     u32 cnt = 0u;                                         // per byte at most 2*WPW <= 8
     if (TW == 1) __syncwarp();            // every lane has its B fragments out of the single buffer
-    Phases<0>::run(r, b, n_tiles, is_obs, ow, cnt, t < T, st_addr + boff, ring_me, ring_next);
+    Phases<0>::run(r, b, n_tiles, is_obs, ow, cnt, t < T, st_addr + boff, st_addr + st_delta + boff, ring_me, ring_next);
     if (is_obs) {
       if (kByteMism) mis += cnt; else mis += __dp4a(cnt, kOnes, 0u);
       ++oj;
@@ -249,7 +269,7 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
       team_sync();
       u32 lo[NW], hi[NW];
       lds_vec(ld_addr + boff, lo);
-      lds_vec(ld_addr + boff + NW * 4, hi);
+      lds_vec(ld_addr + boff + (SWZ ? 512 : NW * 4), hi);
 #pragma unroll
       for (int i = 0; i < NW; ++i) { b[i] = lo[i]; b[NW + i] = hi[i]; }
     }

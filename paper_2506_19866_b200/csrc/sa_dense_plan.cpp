@@ -101,7 +101,7 @@ bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::ve
 }  // namespace
 
 void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& pl, int team_warps, bool want_sparse,
-                      DensePlan* dp) {
+                      bool want_swizzle, DensePlan* dp) {
   *dp = DensePlan();
   const int N = pl.N, E = pl.E, K = pl.K, NO = pl.n_obs;
   if (N > 128) { dp->why = "more than 128 nodes"; return; }
@@ -117,6 +117,8 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   dp->MT = MT; dp->KS = KS; dp->W = W;
   pick_strides(KS, W, &dp->CS, &dp->TS, &dp->exchange_wavefronts);
   const int CS = dp->CS, TS = dp->TS;
+  dp->swizzle = want_swizzle && KS == 4 && W == 1;
+  if (dp->swizzle) dp->exchange_wavefronts = 16;
 
   // Row r = 16m + 8h + g is produced by thread group g as byte j of its word w, q = 2m + h = 4w + j.
   // That byte is stored at chunk t' = g % 4, word pos = (g / 4) * NW + w, which B-fragment thread t'
@@ -141,6 +143,8 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   for (int i = 0; i < N; ++i) { node_of_row[row_of_node[i]] = i; node_of_col[col_of_row(row_of_node[i])] = i; }
   auto state_offset = [&](int cond, int node) {     // byte of (cond, node) in the exchange buffer
     const int k = col_of_row(row_of_node[node]), pos = k / 16, tq = (k % 16) / 4, j = k % 4;
+    if (dp->swizzle)                                 // see the kernel: row 4*half + c/2, column from a Latin square
+      return (4 * (pos / 4) + cond / 2) * 128 + (4 * (tq & 1) + ((cond / 2 + 2 * (tq / 2) + (cond & 1)) & 3)) * 16 + (pos % 4) * 4 + j;
     return cond * CS + tq * TS + pos * 4 + j;
   };
   std::map<std::pair<int, int>, int> edge_at;       // (dst, src) -> edge

@@ -15,6 +15,7 @@ struct DensePlan {
   bool ok = false;
   std::string why;          // reason when !ok
   int MT = 0, KS = 0;       // 16-row tiles, 32-column steps (KS = result words per condition and thread group)
+  bool swizzle = false;     // swizzled exchange buffer (KS = 4, one warp per chain): 16 instead of 24 wavefronts per exchange
   bool sparse = false;      // 2:4-sparse A operand (mma.sp m16n8k64): nodes permuted so that every row has <= 2 candidates per 4 columns
   int W = 1;                // warps per chain; warp ww owns result words ww*KS/W .. and their row tiles
   int CS = 0, TS = 0;       // byte strides of the exchange buffer: per condition, per B-fragment thread chunk
@@ -30,13 +31,13 @@ struct DensePlan {
   std::vector<uint32_t> wloc;        // [E]
   std::vector<uint32_t> thloc;       // [N]
   size_t smem_bytes(const Plan& pl) const {   // per chain, as CHAIN_SMEM in the kernel
-    return ((size_t)(W > 1 ? 2 : 1) * 8 * CS + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 2) * 4 + 15) / 16 * 16;
+    return ((size_t)(W > 1 ? 2 : 1) * (swizzle ? 1024 : 8 * CS) + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 2) * 4 + 15) / 16 * 16;
   }
 };
 
 // Applies when N <= 128 and K <= 8.  team_warps = warps per chain (1, 2 or 4; reduced until it
 // divides KS).  Always returns; check dp->ok / dp->why.
 void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& plan, int team_warps, bool want_sparse,
-                      DensePlan* dp);
+                      bool want_swizzle, DensePlan* dp);
 
 }  // namespace tsa

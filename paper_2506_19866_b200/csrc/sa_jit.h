@@ -22,6 +22,7 @@ struct StaticTuning {
                           // registers) with the sparse A operand, 12 (168 registers) with the dense one
   int dense_phases = 1;   // dense kernel: phases of a time step (accumulator tiles live at a time = row tiles / phases)
   int dense_cpb = 1;      // dense kernel: one-warp chains per CTA (1, 4, 8 or 12); > 1 turns the tensor-pipe token ring on
+  int dense_swizzle = 1;  // dense kernel: swizzled exchange buffer when it applies
   int dense_sparse = 1;   // dense kernel: use the 2:4-sparse A operand (mma.sp) when the network allows it
   int dense_warps = 1;    // dense kernel: warps per chain (1, 2 or 4); 1 measured fastest at every R
   static StaticTuning from_env();
