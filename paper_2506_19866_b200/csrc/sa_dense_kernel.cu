@@ -1,4 +1,4 @@
-// sa_run kernel v4 (sm_100a), for networks of at most 128 nodes and 8 conditions: the node update
+// sa_run kernel v4 / v5 (sm_100a), for networks of at most 128 nodes and 8 conditions: the node update
 // of one time step is ONE dense int8 product on the tensor pipe instead of E shared-memory gathers,
 //
 //     sum[i][k] = SUM_j  W[i][j] * s[j][k]      (PAPER.md :66-70: the image of node i is a sum over its sources)
@@ -8,7 +8,9 @@
 // TW warps = one CTA; warp ww owns the row tiles of its NW/TW result words.  The team keeps the WHOLE
 // of W in registers as mma.sync m16n8k32 A fragments (up to 2*NW/TW*KS*4 registers per thread) for
 // the entire sa_run, every warp the states of t-1 as KS B fragments, and the team issues MT*KS IMMAs
-// per time step.  The sums come back as C fragments, are packed four to a word (byte lanes), thresholded with
+// per time step (v5: the 2:4-sparse form, mma.sp m16n8k64 -- half the registers and half the IMMAs; the
+// host permutes the nodes so that every row has at most two candidate edges per four columns).
+// The sums come back as C fragments, are packed four to a word (byte lanes), thresholded with
 // the same biased-byte trick as the gather kernel, and go through a 1-2 KB shared-memory buffer laid
 // out so that every lane writes its result words with one vector store and reads its next B
 // fragments with two vector loads (row <-> column numbering chosen by the host, sa_dense_plan.cpp).

@@ -90,7 +90,7 @@ bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::ve
     if (after <= before) {                 // rows fed by both a and b are counted twice on both sides
       node_at[r2] = a; node_at[ra] = b;
       cost = 0;
-      if (after != before) for (int i = 0; i < N; ++i) cost += row_cost(i); else for (int i = 0; i < N; ++i) cost += row_cost(i);
+      for (int i = 0; i < N; ++i) cost += row_cost(i);
     } else {
       row[a] = ra; if (b >= 0) row[b] = r2;
     }
