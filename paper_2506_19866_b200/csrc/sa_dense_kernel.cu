@@ -41,6 +41,7 @@
 #define TSD_REDERIVE 1
 #define TSD_SP 1
 #define TSD_SWZ 1
+#define TSD_EARLY_OBS 0
 #endif
 
 namespace tsa_dense {
@@ -185,6 +186,13 @@ struct Phases {
           if (TW * MTW <= MT || 2 * W0 + mi < n_tiles) imma(acc[mi], &r.A[((2 * W0 + mi) * KS + s) * 4], b[2 * s], b[2 * s + 1]);
     }
     if (CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
+    u32 ov[2][WPP];                                      // observation words, in flight while the sums are packed
+    if (TSD_EARLY_OBS && is_obs) {
+#pragma unroll
+      for (int c = 0; c < 2; ++c)
+#pragma unroll
+        for (int w = 0; w < WPP; ++w) ov[c][w] = __ldg(ow + c * NW + W0 + w);
+    }
     u32 ns[2][WPP];
 #pragma unroll
     for (int w = 0; w < WPP; ++w)
@@ -201,7 +209,7 @@ struct Phases {
       for (int c = 0; c < 2; ++c)
 #pragma unroll
         for (int w = 0; w < WPP; ++w) {
-          const u32 z = ns[c][w] ^ __ldg(ow + c * NW + W0 + w);
+          const u32 z = ns[c][w] ^ (TSD_EARLY_OBS ? ov[c][w] : __ldg(ow + c * NW + W0 + w));
           cnt += (z | (z >> 1)) & kOnes;
         }
     }
@@ -342,8 +350,8 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
   // on only if every member has a chain; then all of them run the same number of time steps
   int ring_me = 0, ring_next = 0;
   if (CPB > 1) {
-    const int q = wc & 3, pos = wc >> 2, G = CPB / 4;
-    if (blockIdx.x * CPB + q + 4 * (G - 1) < (u32)p.R) {
+    const int q = wc & 3, pos = wc >> 2, G = CPB >= 4 ? CPB / 4 : 1;
+    if (blockIdx.x * CPB + (u32)(q + 4 * (G - 1)) < (u32)p.R) {
       ring_me = 1 + wc;
       ring_next = 1 + q + 4 * ((pos + 1) % G);
       if (pos == G - 1) ring_pass(ring_next);                        // the token starts at the ring's first warp

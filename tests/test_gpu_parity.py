@@ -313,6 +313,24 @@ def test_balanced_slots_hand_chains_over(B, problems_cache):
     assert np.array_equal(balanced[0], plain[0]) and np.array_equal(balanced[1], plain[1])
 
 
+def test_sparse_operand_applies_or_falls_back(B):
+    """The 2:4-sparse A operand needs at most two candidate edges per row in every group of four
+    columns after the host's node permutation: sparse networks get it, a candidate graph that is 60 %
+    full cannot, and AUTO then runs the dense operand.  Same results either way."""
+    for name, N, E, want_sparse in (("sp_ok", 60, 420, 1), ("sp_full", 40, 940, 0)):
+        cs = PB.ConfigSpec(name, 31 + N, N, E, "uniform-pairs", 6, 2, 8, (4, 8), 8, 150, max_in_degree=39)
+        prob = PB.make_problem(name, O.simulate_fn, spec=cs, noise=0.05)
+        orc = O.Oracle(prob)
+        sched = PB.make_schedule(8, 150)
+        with Handle(B, prob, sched) as hd:
+            B.sa_select_kernel(hd.h, B.SA_KERNEL_DENSE)
+            B.sa_set_trace(hd.h, list(range(8)), 150)
+            B.sa_run(hd.h, 150)
+            di = B.sa_get_dense_info(hd.h)
+            assert di["applies"] == 1 and di["sparse"] == want_sparse, di
+            check_chains(B, hd, orc, list(range(8)), 150, B.sa_get_trace(hd.h, 8, 150))
+
+
 def test_dense_kernel_limits(B):
     """The dense family applies up to 128 nodes and 8 conditions; beyond that DENSE fails loudly
     and AUTO falls back to the gather kernels with identical results."""
