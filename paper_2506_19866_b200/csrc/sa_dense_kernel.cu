@@ -42,6 +42,7 @@
 #define TSD_SP 1
 #define TSD_SWZ 1
 #define TSD_EARLY_OBS 0
+#define TSD_TUNROLL 1
 #endif
 
 namespace tsa_dense {
@@ -58,6 +59,7 @@ constexpr bool SP = TSD_SP != 0;                // 2:4-sparse A operand: mma.sp 
 constexpr int KSP = KS / 2;                     // sparse steps of 64 columns
 constexpr int NA = SP ? MTW * KSP * 4 : MTW * KS * 4;   // A-fragment registers per thread
 constexpr int NM = SP ? MTW * KSP : 1;          // selector (metadata) registers per thread
+constexpr int kTUnroll = TSD_TUNROLL;           // unroll factor of the time loop
 constexpr bool SWZ = TSD_SWZ != 0;              // swizzled exchange buffer (KS = 4, one warp per chain): conflict-free stores AND loads
 constexpr int STATE_BYTES = SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
@@ -259,7 +261,7 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
   }
   u32 mis = 0u;
   int oj = 0;
-#pragma unroll 1
+#pragma unroll (kTUnroll)
   for (int t = 1; t <= T; ++t) {
     const bool is_obs = t < 64 ? ((kObsLo >> t) & 1ull) : ((kObsHi >> (t - 64)) & 1ull);
     const u32* ow = p.obs_word + ((size_t)oj * 32 + lane) * (2 * NW) + ww * WPW;
