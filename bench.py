@@ -242,7 +242,7 @@ def run_ours(args) -> dict:
             "roofline": {"bound": "alu", "achieved": achieved / 1e12, "peak": issue_peak / 1e12,
                          "unit": "T int-lane-op/s", "frac": achieved / issue_peak,
                          # dram__bytes_read.sum + dram__bytes_write.sum of one sa_run launch, from the ncu capture in
-                         # profiles/r1_v5_run_dense_sparse_kernel.md (stage + write back of the chains; HBM is not the bound)
+                         # profiles/r1_v6_run_dense_sparse_unrolled.md (stage + write back of the chains; HBM is not the bound)
                          "traffic": 6.10e6 if name == "mtb" else None,
                          "peak_source": f"{sms} SMs x 4 schedulers x 32 lanes x {sm_max_hz/1e6:.0f} MHz "
                                         "(MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §7)",
