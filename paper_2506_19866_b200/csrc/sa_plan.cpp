@@ -384,7 +384,7 @@ int build_plan(const sa_network* net, const sa_observations* obs, bool need_obs,
     std::vector<int> order(np0);
     std::iota(order.begin(), order.end(), 0);
     std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return best_iters[a] > best_iters[b]; });
-    const int max_slots = opt.max_lane_slots > 0 ? opt.max_lane_slots : (CG == 4 ? 40 : 48);
+    const int max_slots = opt.max_lane_slots > 0 ? opt.max_lane_slots : (CG == 4 ? 64 : 48);   // Large: 64 -> 8 warps per chain, 3.47 M (40: 16 warps, 3.30 M)
     // W is a power of two (a 128-register budget then fills an SM's 512 threads with whole teams)
     int w_lo = 1;
     while (w_lo < std::min(opt.min_team_warps, 32) && 2 * w_lo <= np0) w_lo *= 2;
