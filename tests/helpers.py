@@ -1,5 +1,8 @@
 """Shared test helpers: hand-specified example networks and golden-file readers."""
+import functools
 import os
+import subprocess
+import tempfile
 
 import numpy as np
 
@@ -59,3 +62,42 @@ def all_settings(n_edges, n_nodes, n_pairs):
         out[:, n_edges + i] = idx % n_pairs
         idx //= n_pairs
     return out
+
+
+_ATEN_SRC = r"""
+#include <ATen/core/PhiloxRNGEngine.h>
+#include <cstdio>
+#include <cstdlib>
+int main() {
+  unsigned long long seed, sub, off;
+  while (scanf("%llu %llu %llu", &seed, &sub, &off) == 3) {
+    at::Philox4_32 eng(seed, sub, off);
+    unsigned r0 = eng(), r1 = eng(), r2 = eng(), r3 = eng();
+    printf("%u %u %u %u\n", r0, r1, r2, r3);
+  }
+  return 0;
+}
+"""
+
+
+@functools.lru_cache(maxsize=1)
+def _aten_philox_exe():
+    """ATen's own Philox4_32 engine compiled into a tiny program: an implementation of Philox4x32-10
+    that is independent of the oracle's and of the CUDA path's (SURVEY.md §8(c) Pin 8)."""
+    import torch
+    inc = os.path.join(os.path.dirname(torch.__file__), "include")
+    td = tempfile.mkdtemp(prefix="aten_philox_")
+    src, exe = os.path.join(td, "p.cpp"), os.path.join(td, "p")
+    with open(src, "w") as f:
+        f.write(_ATEN_SRC)
+    subprocess.check_call(["g++", "-O1", "-std=c++17", "-I", inc, src, "-o", exe])
+    return exe
+
+
+def aten_philox_blocks(cases):
+    """cases: (seed, subsequence, offset) triples -> one [r0, r1, r2, r3] block each, from
+    at::Philox4_32(seed, subsequence, offset).  Correspondence with the method's counter layout:
+    subsequence = chain | domain << 32, offset = step g (checked by test_philox_matches_aten_engine)."""
+    text = "".join(f"{s} {sub} {off}\n" for s, sub, off in cases)
+    out = subprocess.check_output([_aten_philox_exe()], input=text.encode()).decode().split("\n")
+    return [[int(v) for v in line.split()] for line in out if line.strip()]

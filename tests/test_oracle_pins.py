@@ -3,16 +3,13 @@ oracle's own formula — they are hand-worked values (tests/golden), closed form
 a dense library-matmul special case and brute force on a tiny network."""
 import copy
 import os
-import subprocess
-import sys
-import tempfile
 
 import numpy as np
 import pytest
 
 from oracle import oracle as O
 from paper_2506_19866_b200 import problems as PB
-from helpers import all_settings, brute_force_problem, example_problem, golden_rows
+from helpers import all_settings, aten_philox_blocks, brute_force_problem, example_problem, golden_rows
 
 
 # ------------------------------------------------------------------ Pin 1 / Pin 2: hand-worked
@@ -300,44 +297,100 @@ def test_brute_force_4_nodes_6_edges():
 
 
 # ------------------------------------------------------------------ Pin 8: Philox vs ATen's engine
-_ATEN_SRC = r"""
-#include <ATen/core/PhiloxRNGEngine.h>
-#include <cstdio>
-#include <cstdlib>
-int main(int argc, char** argv) {
-  for (int a = 1; a + 2 < argc; a += 3) {
-    unsigned long long seed = strtoull(argv[a], 0, 0), sub = strtoull(argv[a+1], 0, 0), off = strtoull(argv[a+2], 0, 0);
-    at::Philox4_32 eng(seed, sub, off);
-    unsigned r0 = eng(), r1 = eng(), r2 = eng(), r3 = eng();
-    printf("%u %u %u %u\n", r0, r1, r2, r3);
-  }
-  return 0;
-}
-"""
-
-
 def test_philox_matches_aten_engine():
-    import torch
-    inc = os.path.join(os.path.dirname(torch.__file__), "include")
     cases = [(42, 0, 0, 0), (42, 7, 0, 123456), (0xDEADBEEFCAFEF00D, 4095, 1, 0x1_0000_0005),
              (1, 0xFFFFFFFF, 1, 0xFFFFFFFF), (0, 0, 0, 1), (42, 65535, 0, 19999)]
-    with tempfile.TemporaryDirectory() as td:
-        src, exe = os.path.join(td, "p.cpp"), os.path.join(td, "p")
-        with open(src, "w") as f:
-            f.write(_ATEN_SRC)
-        subprocess.check_call(["g++", "-O1", "-std=c++17", "-I", inc, src, "-o", exe])
-        args = []
-        for seed, chain, domain, g in cases:
-            args += [str(seed), str(chain | (domain << 32)), str(g)]
-        out = subprocess.check_output([exe] + args).decode().split("\n")
-    for (seed, chain, domain, g), line in zip(cases, out):
-        want = [int(v) for v in line.split()]
+    blocks = aten_philox_blocks([(seed, chain | (domain << 32), g) for seed, chain, domain, g in cases])
+    for (seed, chain, domain, g), want in zip(cases, blocks):
         got = O.philox4x32_10([g & 0xFFFFFFFF, g >> 32, chain, domain], [seed & 0xFFFFFFFF, seed >> 32])
         assert got == want, (seed, chain, domain, g)
     # counters differing in one word give unrelated blocks
     a = O.philox4x32_10([0, 0, 0, 0], [42, 0])
     for ctr in ([1, 0, 0, 0], [0, 1, 0, 0], [0, 0, 1, 0], [0, 0, 0, 1]):
         assert O.philox4x32_10(ctr, [42, 0]) != a
+
+
+# ------------------------------------------------------------------ the wiring of one chain step
+def _level_gated_table(n_levels, dmax):
+    """Row l accepts a worse move with probability 1/2 iff d <= l (threshold 2^31 up to d = l, 0
+    beyond): rows differ strongly by level, so a level index that is off by one or does not saturate
+    changes decisions, and the decision depends on the value of x2, so another word in its place does too."""
+    tab = np.zeros((n_levels, dmax), dtype=np.uint32)
+    for l in range(n_levels):
+        tab[l, :min(l, dmax)] = 0x80000000
+    return tab
+
+
+@pytest.mark.parametrize("name,chain,g0", [("tiny", 3, 0), ("hpg", 5, 0), ("tiny", 2, (1 << 32) - 60)])
+def test_chain_step_wiring_recomputed_outside_the_oracle(problems_cache, name, chain, g0):
+    """SURVEY.md §8(c)-3 / PAPER.md Table 1 :130-149, recomputed step by step OUTSIDE orc_run_chain
+    from independently pinned pieces: the random block from ATen's Philox engine (seed, subsequence =
+    chain | 0 << 32, offset = g), the index and the new value by integer arithmetic written here,
+    delta_cand from Oracle.fitness (Pins 1, 2, 5, 7), level = min(g // spl, L-1), accept iff d <= 0 or
+    (d <= D and x2 < table[level][d-1]).  Fails if orc_run_chain swaps counter words, uses domain 1,
+    feeds x1 / x3 to the accept test, is off by one in the level or does not saturate it."""
+    prob = problems_cache(name)
+    orc = O.Oracle(prob)
+    E, NP, n_pairs = prob.n_edges, prob.n_params, prob.n_pairs
+    L, spl, D, n = 8, 20, 6, 230                                      # L * spl = 160 < 230: 70 saturated steps
+    sched = PB.make_schedule(8, L * spl, n_levels=L, dmax=D)
+    sched.accept = _level_gated_table(L, D)
+    assert sched.steps_per_level == spl
+    cur, f0 = orc.init_chain(sched.seed, chain)
+    state = None
+    if g0:                                                           # start far along: g no longer fits 32 bits midway
+        state = (cur, cur.copy(), f0, f0)
+    run = orc.run_chain(sched, chain, n, g0=g0, state=state)
+    tr = O.unpack_trace(run["trace"])
+    blocks = aten_philox_blocks([(sched.seed, chain, g0 + it) for it in range(n)])
+    x = cur.copy()
+    best, fc, fb = x.copy(), f0, f0
+    seen_levels, gated = set(), 0
+    for it in range(n):
+        g = g0 + it
+        x0, x1, x2, _x3 = blocks[it]
+        p = (x0 * NP) >> 32
+        if p < E:
+            nv = (int(x[p]) + 1 + 1 + ((x1 * 2) >> 32)) % 3 - 1
+        else:
+            nv = (int(x[p]) + 1 + ((x1 * (n_pairs - 1)) >> 32)) % n_pairs
+        cand = x.copy()
+        cand[p] = nv
+        fcand = orc.fitness(cand)
+        d = fcand - fc
+        level = min(g // spl, L - 1)
+        acc = d <= 0 or (d <= D and x2 < int(sched.accept[level][d - 1]))
+        if 0 < d <= D:
+            gated += 1
+            seen_levels.add(level)
+        new_best = acc and fcand < fb
+        assert int(tr["param"][it]) == p, (it, "parameter index")
+        assert int(tr["code"][it]) == (nv + 1 if p < E else nv), (it, "new value")
+        assert int(tr["delta_cand"][it]) == fcand, (it, "candidate fitness")
+        assert bool(tr["accepted"][it]) == acc, (it, "accept decision", d, level)
+        assert bool(tr["new_best"][it]) == new_best, (it, "new best")
+        if acc:
+            x, fc = cand, fcand
+            if new_best:
+                best, fb = cand.copy(), fcand
+    assert np.array_equal(x, run["cur"]) and np.array_equal(best, run["best"])
+    assert (fc, fb) == (run["fit_cur"], run["fit_best"])
+    if g0 == 0:
+        assert gated >= 20 and len(seen_levels) >= 4                  # the level-dependent branch was exercised
+    else:
+        assert g0 + n > (1 << 32)                                     # the high counter word was exercised
+
+
+def test_accept_boundaries():
+    """d == D is still looked up (last column), d == D + 1 is rejected whatever the row holds."""
+    D = 6
+    ones = np.full(D, 0xFFFFFFFF, dtype=np.uint32)
+    assert O.accept(D, 0, ones) is True and O.accept(D, 0xFFFFFFFE, ones) is True
+    assert O.accept(D, 0xFFFFFFFF, ones) is False                    # strict <
+    assert O.accept(D + 1, 0, ones) is False
+    last_only = np.zeros(D, dtype=np.uint32); last_only[D - 1] = 7
+    assert O.accept(D, 6, last_only) is True and O.accept(D, 7, last_only) is False
+    assert O.accept(D - 1, 0, last_only) is False                    # column d-1, not d
 
 
 def test_chain_init_uses_domain_1(problems_cache):
