@@ -379,3 +379,220 @@ def spread_chains(n_chains: int, count: int, head: int = 4) -> List[int]:
     for k in range(rest):
         ids.append(min(n_chains - 1, head + ((n_chains - head) * k) // max(rest, 1)))
     return sorted(set(ids))
+
+
+# =========================================================================== paper model
+# Inputs for the paper's OWN model (§2.1-2.3, §2.5): three
+# parameters per edge (w, p, t), three per node (u, m, d), one time course of T+1 points per
+# condition, a reference matrix R with 255 = entity not measured.  As above, nothing here updates a
+# state or scores a trajectory: the ground-truth time course comes from the injected callback.
+
+@dataclass(frozen=True)
+class PaperSpec:
+    name: str
+    seed: int
+    n_nodes: int
+    n_edges: int
+    n_measured: int
+    n_fast: int
+    n_cond: int
+    n_steps: int             # T transitions = T+1 time points including t0
+    noise: float
+    n_chains: int
+    sa_steps: int
+
+
+# The paper's two systems by SHAPE (their edge lists and data are not in the container): HPG axis
+# 9 nodes / 25 edges / 102 parameters, 5 of 9 measured, FSH / GNRH1 / LH fast, 20 time points,
+# experimental (hence imperfectly fitting) data; Mtb 63 / 178 / 723, 35
+# measured, one third fast, 20 time points, self-generated noise-free data (:182-184).
+PAPER_CONFIGS: Dict[str, PaperSpec] = {
+    "paper_tiny": PaperSpec("paper_tiny", 2001, 5, 11, 3, 2, 2, 9, 0.05, 8, 2000),
+    "paper_hpg": PaperSpec("paper_hpg", 2002, 9, 25, 5, 3, 1, 19, 0.05, 10240, 5000),
+    "paper_mtb": PaperSpec("paper_mtb", 2003, 63, 178, 35, 21, 1, 19, 0.0, 10240, 5000),
+}
+PAPER_T0, PAPER_TMIN, PAPER_RHO, PAPER_ITERS = 1000.0, 0.001, 0.99, 5000
+
+
+@dataclass
+class PaperProblem:
+    name: str
+    seed: int
+    n_nodes: int
+    n_edges: int
+    edge_src: np.ndarray      # int32 [E]
+    edge_dst: np.ndarray      # int32 [E]
+    fast: np.ndarray          # uint8 [N] 1 = speed range {10,11,12}, 0 = {1..6}
+    n_cond: int
+    n_steps: int              # T
+    init_state: np.ndarray    # uint8 [K][N]
+    ref: np.ndarray           # uint8 [K][T+1][N] in {0,1,2} or 255
+    truth: Optional[np.ndarray] = None
+    ref_clean: Optional[np.ndarray] = None
+    measured_nodes: Optional[np.ndarray] = None
+    n_flipped: int = 0
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def n_params(self) -> int:
+        return 3 * self.n_edges + 3 * self.n_nodes
+
+    @property
+    def n_scored(self) -> int:
+        return int((self.ref != UNOBSERVED).sum())
+
+    @property
+    def max_objective(self) -> int:
+        """Upper bound of y: |S-R| <= 2 and |G|+1 <= 3 per measured entry."""
+        return 6 * self.n_scored
+
+    @property
+    def node_updates_per_step(self) -> int:
+        return self.n_cond * self.n_steps * self.n_nodes
+
+    @property
+    def alg_ops_per_step(self) -> int:
+        """Scalar integer operations one chain-step must do: per transition one
+        multiply-add per edge (image) and 8 per node (clip, compare, memory test, priority product,
+        maximum, equality with the maximum, bounded move, counter update), plus one
+        absolute-difference-multiply-add per measured entry of every time point."""
+        return self.n_cond * self.n_steps * (self.n_edges + 8 * self.n_nodes) + self.n_scored
+
+    def layout(self):
+        """Offsets of w, p, t, u, m, d in the parameter vector."""
+        e, n = self.n_edges, self.n_nodes
+        return {"w": 0, "p": e, "t": 2 * e, "u": 3 * e, "m": 3 * e + n, "d": 3 * e + 2 * n}
+
+
+def paper_domain(prob: PaperProblem, q: int):
+    """Values parameter q may take, in increasing order."""
+    e, n = prob.n_edges, prob.n_nodes
+    if q < e:
+        return (0, 1, 2)
+    if q < 2 * e:
+        return (-1, 0, 1)
+    if q < 3 * e:
+        return (1, 2)
+    q -= 3 * e
+    if q < n:
+        return (10, 11, 12) if prob.fast[q] else (1, 2, 3, 4, 5, 6)
+    if q < 2 * n:
+        return (0, 1, 2)
+    return (1, 2)
+
+
+def paper_schedule(n_chains: int, n_levels: int, steps_per_level: int, dmax: int, seed: int = SA_SEED,
+                   t0: float = PAPER_T0, rho: float = PAPER_RHO, chain_id_base: int = 0) -> Schedule:
+    """The paper's cooling T_l = t0 * rho^l as an integer acceptance table
+    floor(2^32 * exp(-d / T_l)), d = 1..dmax.  The full schedule is 1375 levels x 5000 iterations
+    (T = 1000 down to 0.001); tests and bench.py run slices of it."""
+    out = np.zeros((n_levels, dmax), dtype=np.uint32)
+    d = np.arange(1, dmax + 1, dtype=np.float64)
+    for l in range(n_levels):
+        temp = t0 * math.pow(rho, l)
+        v = np.floor(4294967296.0 * np.exp(-d / temp))
+        out[l] = np.minimum(v, 4294967295.0).astype(np.uint32)
+    return Schedule(n_chains, seed, n_levels, steps_per_level, dmax, out, n_levels * steps_per_level, chain_id_base)
+
+
+def paper_levels(t0: float = PAPER_T0, tmin: float = PAPER_TMIN, rho: float = PAPER_RHO) -> int:
+    """Number of passes of `while T > Tmin`: 1375 for the paper's constants."""
+    n, t = 0, t0
+    while t > tmin:
+        n += 1
+        t *= rho
+    return n
+
+
+PaperSimulateFn = Callable[[PaperProblem, np.ndarray], np.ndarray]
+"""simulate(problem, params int8[3E+3N]) -> uint8 [K][T+1][N]: the whole time course, t0 included."""
+
+
+def make_paper_problem(name: str, simulate: PaperSimulateFn, seed: Optional[int] = None,
+                       spec: Optional[PaperSpec] = None) -> PaperProblem:
+    spec = spec or PAPER_CONFIGS[name]
+    seed = spec.seed if seed is None else seed
+    n, e, kc, T = spec.n_nodes, spec.n_edges, spec.n_cond, spec.n_steps
+
+    # candidate structure: every node has an in- and an out-edge (closed loop, PAPER.md:187-191)
+    shape = ConfigSpec(spec.name, seed, n, e, "poisson", kc, 0, T, (), 0, 0)
+    src, dst = _make_edges(shape, SplitMix64(seed, 1))
+
+    rng = SplitMix64(seed, 2)
+    init = np.zeros((kc, n), dtype=np.uint8)
+    for k in range(kc):
+        for i in range(n):
+            init[k, i] = rng.below(3)
+    fast = np.zeros(n, dtype=np.uint8)
+    for i in SplitMix64(seed, 3).sample_distinct(n, spec.n_fast):
+        fast[i] = 1
+
+    prob = PaperProblem(name=spec.name, seed=seed, n_nodes=n, n_edges=e, edge_src=src, edge_dst=dst, fast=fast,
+                        n_cond=kc, n_steps=T, init_state=init,
+                        ref=np.full((kc, T + 1, n), UNOBSERVED, dtype=np.uint8))
+
+    # hidden ground truth: uniform over the value ranges, made constraint-compliant by giving every
+    # node one activating in-edge and one non-zero out-edge (PAPER.md:184 "randomized within their
+    # specified ranges ... adhere to the network constraints"); resampled (<= 100 tries) until
+    # >= 30 % of the nodes have a non-constant time course
+    rng = SplitMix64(seed, 4)
+    in_edges = [[k for k in range(e) if dst[k] == i] for i in range(n)]
+    out_edges = [[k for k in range(e) if src[k] == i] for i in range(n)]
+    best_frac, truth, states = -1.0, None, None
+    for attempt in range(100):
+        cand = np.zeros(3 * e + 3 * n, dtype=np.int8)
+        for q in range(3 * e + 3 * n):
+            dom = paper_domain(prob, q)
+            cand[q] = dom[rng.below(len(dom))]
+        for i in range(n):
+            k = in_edges[i][rng.below(len(in_edges[i]))]
+            cand[e + k] = 1
+            cand[k] = max(int(cand[k]), 1)
+        for i in range(n):
+            if not any(cand[k] > 0 for k in out_edges[i]):
+                cand[out_edges[i][rng.below(len(out_edges[i]))]] = 1
+        st = np.asarray(simulate(prob, cand), dtype=np.uint8).reshape(kc, T + 1, n)
+        dynamic = (st.max(axis=1) != st.min(axis=1)).any(axis=0)
+        frac = float(dynamic.mean())
+        if frac > best_frac:
+            best_frac, truth, states = frac, cand, st
+        if frac >= 0.30:
+            break
+    prob.truth = truth
+    prob.meta["dynamic_fraction"] = best_frac
+    prob.meta["truth_attempts"] = attempt + 1
+
+    # measured subset: dynamic nodes first, then the others, each group in random order (:184 "mostly
+    # randomly selected; however, we prioritize ... a more dynamic time course")
+    rng = SplitMix64(seed, 5)
+    dynamic = (states.max(axis=1) != states.min(axis=1)).any(axis=0)
+    order = rng.sample_distinct(n, n)
+    ranked = [i for i in order if dynamic[i]] + [i for i in order if not dynamic[i]]
+    measured = np.array(sorted(ranked[:spec.n_measured]), dtype=np.int32)
+    prob.measured_nodes = measured
+    clean = np.full((kc, T + 1, n), UNOBSERVED, dtype=np.uint8)
+    clean[:, :, measured] = states[:, :, measured]
+    prob.ref_clean = clean
+
+    rng = SplitMix64(seed, 6)
+    noisy = clean.copy()
+    n_entries = kc * (T + 1) * len(measured)
+    n_flip = int(round(spec.noise * n_entries))
+    for code in rng.sample_distinct(n_entries, n_flip):
+        k, rem = divmod(code, (T + 1) * len(measured))
+        t, oi = divmod(rem, len(measured))
+        i = int(measured[oi])
+        noisy[k, t, i] = (int(noisy[k, t, i]) + 1 + rng.below(2)) % 3
+    prob.ref = noisy
+    prob.n_flipped = n_flip
+    return prob
+
+
+def random_paper_params(prob: PaperProblem, count: int, seed: int) -> np.ndarray:
+    """count i.i.d. uniform parameter vectors int8 [count][3E+3N] (inputs for sap_eval parity)."""
+    rng = np.random.Generator(np.random.Philox(seed))
+    out = np.zeros((count, prob.n_params), dtype=np.int8)
+    for q in range(prob.n_params):
+        dom = np.array(paper_domain(prob, q), dtype=np.int8)
+        out[:, q] = dom[rng.integers(0, len(dom), size=count)]
+    return out
