@@ -173,6 +173,94 @@ int sa_jit_check(const sa_network *net, const sa_observations *obs, int32_t n_ch
  * obs->obs may be NULL.  Fails like sa_create on invalid input. */
 int sa_plan_info(const sa_network *net, const sa_observations *obs, int64_t info[16]);
 
+/* ==================================================================================================
+ * The paper's OWN model: three parameters
+ * per edge and per node, the priority update scheme, the gradient-weighted objective, the structural
+ * constraints, acceptance statistics per temperature level.  Same chain step (Table 1), same
+ * Philox counter layout, same integer accept test and same trace records as above.
+ *
+ * Parameter vector everywhere below: int8 params[3E+3N] = [w(E), p(E), t(E), u(N), m(N), d(N)]
+ * (PAPER.md:106-108), the values themselves: w in {0,1,2} weight, p in {-1,0,1} polarity, t in {1,2}
+ * activation threshold of edge e in the caller's edge order (:61-64); u speed in {1..6} (slow node) or
+ * {10,11,12} (fast node), m memory in {0,1,2}, d step size in {1,2} of node i (:78-80).
+ * ================================================================================================== */
+
+typedef struct sap_handle sap_handle;            /* opaque, owned by the library */
+
+typedef struct {
+  int32_t n_nodes, n_edges;                      /* N <= 256, E */
+  const int32_t *edge_src, *edge_dst;            /* [E], no self-loops, no duplicate (src,dst) */
+  const uint8_t *fast;                           /* [N] 1 = speed range {10,11,12}, 0 = {1..6} */
+} sap_network;
+
+/* Time courses: K independent courses (the paper has one), each T transitions =
+ * T+1 time points including t0. */
+typedef struct {
+  int32_t n_cond, n_steps;                       /* K, T (T <= 4095) */
+  const uint8_t *init_state;                     /* [K][N] in {0,1,2}: state at t0 */
+  const uint8_t *ref;                            /* [K][T+1][N] reference matrix R in {0,1,2}, SA_UNOBSERVED = entity
+                                                    not measured; may be NULL for sap_simulate only */
+} sap_observations;
+
+#define SAP_CONSTRAINED 1u   /* structural constraints of PAPER.md:186-201 in GetCandidate and at initialisation */
+#define SAP_LEVEL_STATS 2u   /* count accepted / accepted-worse / new-best moves per temperature level */
+
+/* Build the device-resident problem, allocate the chain store ([R][pitch] int8 in HBM, caller's parameter
+ * order), give every chain its initial vector (Philox domain 1; with SAP_CONSTRAINED followed by the
+ * repair pass of DESIGN.md reading P6, Philox domain 2, so that every chain starts from a valid
+ * vector) and evaluate it.  sched is the same structure as for sa_create; dmax should be
+ * at least the largest objective (6 per measured entry) if no worse move is to be rejected outright.
+ * Validation (SA_EINVAL): counts > 0, N <= 256, T <= 4095, endpoints in range, no self-loop / duplicate
+ * edge, fast in {0,1}, states in {0,1,2}, ref in {0,1,2,255}, at most 256 edge slots per lane
+ * (in-degrees), and with SAP_CONSTRAINED an in-edge and an out-edge at every node. */
+int sap_create(const sap_network *net, const sap_observations *obs, const sa_schedule *sched, uint32_t flags,
+               sap_handle **out);
+
+/* Advance every chain by `steps` SA steps (Table 1 :130-149): GetCandidate (uniform
+ * parameter index; new value uniform over the parameter's other values, with SAP_CONSTRAINED over
+ * those that keep constraints (a) and (b), a null move if there is none), Simulate (priority update
+ * scheme §2.2, objective §2.3), integer Metropolis test, commit.  Asynchronous on the handle's stream. */
+int sap_run(sap_handle *h, int64_t steps);
+
+/* Table 1 with its level synchronisation on the device, as sa_run_levels. */
+int sap_run_levels(sap_handle *h, int64_t n_levels, int32_t group_size);
+
+int sap_best(sap_handle *h, uint32_t *fitness, int32_t *chain, int8_t *params /* [3E+3N] */);
+void sap_destroy(sap_handle *h);
+
+/* Objective y = SUM |S - R| (.) (|G| + 1) of n given vectors, params [n][3E+3N]. */
+int sap_eval(sap_handle *h, const int8_t *params, int64_t n, uint32_t *fitness);
+
+/* Simulate one vector: states [K][T+1][N], t0 included.  Needs no handle. */
+int sap_simulate(const sap_network *net, const sap_observations *obs, const int8_t *params, uint8_t *states);
+
+int sap_get_chain(sap_handle *h, int32_t chain, int8_t *cur, uint32_t *cur_fit, int8_t *best, uint32_t *best_fit);
+int sap_get_fitness(sap_handle *h, uint32_t *cur_fit, uint32_t *best_fit);
+
+/* Trace as sa_set_trace / sa_get_trace.  Record: bits 0-31 delta_cand, 32-55 parameter index, 56-59 index
+ * of the new value in the parameter's range (increasing order), bit 60 accepted, bit 61 new best, bit 62
+ * null move (no value of the parameter keeps the constraints; the candidate is the current vector). */
+int sap_set_trace(sap_handle *h, const int32_t *chains, int32_t n, int64_t max_steps);
+int sap_get_trace(sap_handle *h, uint64_t *records);
+
+/* Acceptance statistics kept on the device (needs SAP_LEVEL_STATS): stats [L][4] = per level of the
+ * schedule (the last one absorbing steps past it), summed over all chains since sap_create: steps,
+ * accepted moves, accepted moves with delta_cand > delta_cur ("worse solutions that are temporarily
+ * accepted"), new bests.  Synchronises the stream. */
+int sap_get_level_stats(sap_handle *h, uint64_t *stats);
+
+/* info[0] = lanes per chain, [1] = node slots per lane, [2] = edge slots per lane, [3] = threads per CTA,
+ * [4] = chains per CTA, [5] = dynamic shared memory bytes per CTA, [6] = CTAs of the sap_run grid,
+ * [7] = registers per thread of the run kernel, [8] = resident CTAs per SM, [9] = SM count,
+ * [10] = kernels launched so far by this handle, [11] = largest objective (6 per measured entry). */
+int sap_get_info(sap_handle *h, int64_t info[12]);
+
+int sap_set_stream(sap_handle *h, void *cuda_stream);
+
+/* Host only (no GPU needed): plan + NVRTC compile of the paper-model kernels for this network.
+ * info[0] = lanes per chain, [1] = node slots, [2] = edge slots, [3] = cubin bytes. */
+int sap_jit_check(const sap_network *net, const sap_observations *obs, int64_t info[4], char *log, size_t log_bytes);
+
 /* ---- plumbing ---- */
 
 /* CUDA stream (cudaStream_t as void*) the handle's kernels and copies run on; default stream 0. */

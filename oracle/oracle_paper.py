@@ -177,3 +177,39 @@ class PaperOracle:
 def simulate_fn(prob, params) -> np.ndarray:
     """The ``simulate`` callback problems.make_paper_problem expects, served by the oracle."""
     return PaperOracle(prob).simulate(params)
+
+
+def run_levels(orc: "PaperOracle", sched, n_chains: int, n_levels: int, group_size: int = 0, g0: int = 0,
+               states=None, threads: int = 1, constrained: bool = False):
+    """PAPER.md Table 1 (:125-155) around the chain step, statement by statement (as oracle.run_levels):
+    per level, n_iterations chain steps of every thread, then per group the smallest d_best (ties: the
+    smallest chain) gives its x_best to every member as x_best and, at the top of the next level (:129),
+    as x_current.  Returns the list of (cur, best, fit_cur, fit_best) after the last level."""
+    R = n_chains
+    group = R if group_size in (0, None) or group_size > R else group_size
+    base = getattr(sched, "chain_id_base", 0)
+    if states is None:
+        states = []
+        for c in range(R):
+            x, f = orc.init_chain(sched.seed, base + c, constrained)
+            states.append((x, x.copy(), f, f))
+    g = g0
+    assert g % sched.steps_per_level == 0, "levels start at level boundaries"
+    for _ in range(n_levels):
+        def advance(c):
+            out = orc.run_chain(sched, base + c, sched.steps_per_level, g0=g, state=states[c], trace=False,
+                                constrained=constrained)
+            return (out["cur"], out["best"], out["fit_cur"], out["fit_best"])
+        if threads > 1:
+            with ThreadPoolExecutor(threads) as ex:
+                states = list(ex.map(advance, range(R)))
+        else:
+            states = [advance(c) for c in range(R)]
+        g += sched.steps_per_level
+        for first in range(0, R, group):
+            members = range(first, min(R, first + group))
+            star = min(members, key=lambda c: (states[c][3], c))
+            x_star, d_star = states[star][1], states[star][3]
+            for c in members:
+                states[c] = (x_star.copy(), x_star.copy(), d_star, d_star)
+    return states

@@ -20,7 +20,11 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info")
+           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info",
+           "sap_create", "sap_run", "sap_run_levels", "sap_best", "sap_destroy", "sap_eval", "sap_simulate",
+           "sap_get_chain", "sap_get_fitness", "sap_set_trace", "sap_get_trace", "sap_get_level_stats", "sap_get_info",
+           "sap_set_stream", "sap_jit_check")
+SAP_CONSTRAINED, SAP_LEVEL_STATS = 1, 2
 SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
 
 if not os.path.exists(LIB_PATH):
@@ -77,6 +81,33 @@ _lib.sa_set_allocator.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_int32_peak.argtypes = [C.c_void_p]
 _lib.sa_select_kernel.argtypes = [C.c_void_p, C.c_int]
 _lib.sa_jit_check.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c_int32, C.c_void_p, C.c_char_p, C.c_size_t]
+
+
+class _PNetwork(C.Structure):
+    _fields_ = [("n_nodes", C.c_int32), ("n_edges", C.c_int32), ("edge_src", C.c_void_p), ("edge_dst", C.c_void_p),
+                ("fast", C.c_void_p)]
+
+
+class _PObservations(C.Structure):
+    _fields_ = [("n_cond", C.c_int32), ("n_steps", C.c_int32), ("init_state", C.c_void_p), ("ref", C.c_void_p)]
+
+
+_lib.sap_create.argtypes = [C.POINTER(_PNetwork), C.POINTER(_PObservations), C.POINTER(_Schedule), C.c_uint32, C.POINTER(C.c_void_p)]
+_lib.sap_run.argtypes = [C.c_void_p, C.c_int64]
+_lib.sap_run_levels.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
+_lib.sap_best.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sap_destroy.argtypes = [C.c_void_p]
+_lib.sap_destroy.restype = None
+_lib.sap_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+_lib.sap_simulate.argtypes = [C.POINTER(_PNetwork), C.POINTER(_PObservations), C.c_void_p, C.c_void_p]
+_lib.sap_get_chain.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sap_get_fitness.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sap_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64]
+_lib.sap_get_trace.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sap_get_level_stats.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sap_get_info.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sap_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+_lib.sap_jit_check.argtypes = [C.POINTER(_PNetwork), C.POINTER(_PObservations), C.c_void_p, C.c_char_p, C.c_size_t]
 
 
 def _check(rc: int, where: str):
@@ -276,3 +307,118 @@ def sa_int32_peak() -> dict:
 def sa_last_error() -> str:
     msg = _lib.sa_last_error()
     return msg.decode() if msg else ""
+
+
+# ------------------------------------------------------------------------------- the paper model
+def _marshal_paper(prob, need_ref: bool = True):
+    keep = {"src": _arr(prob.edge_src, np.int32), "dst": _arr(prob.edge_dst, np.int32), "fast": _arr(prob.fast, np.uint8),
+            "init": _arr(prob.init_state, np.uint8)}
+    net = _PNetwork(prob.n_nodes, prob.n_edges, keep["src"].ctypes.data, keep["dst"].ctypes.data, keep["fast"].ctypes.data)
+    ref_ptr = None
+    if need_ref:
+        keep["ref"] = _arr(prob.ref, np.uint8)
+        ref_ptr = keep["ref"].ctypes.data
+    obs = _PObservations(prob.n_cond, prob.n_steps, keep["init"].ctypes.data, ref_ptr)
+    return net, obs, keep
+
+
+def sap_create(prob, sched, flags: int = 0, stream: Optional[int] = None) -> int:
+    """prob / sched: objects with the fields of problems.PaperProblem / problems.Schedule.  Returns the handle."""
+    net, obs, keep = _marshal_paper(prob)
+    table = _arr(sched.accept, np.uint32)
+    sc = _Schedule(sched.n_chains, sched.seed, sched.n_levels, sched.steps_per_level, sched.dmax,
+                   table.ctypes.data, getattr(sched, "chain_id_base", 0))
+    h = C.c_void_p()
+    _check(_lib.sap_create(C.byref(net), C.byref(obs), C.byref(sc), flags, C.byref(h)), "sap_create")
+    if stream is None and _hooks is not None:
+        import torch
+        stream = torch.cuda.current_stream().cuda_stream
+    if stream:
+        _check(_lib.sap_set_stream(h, C.c_void_p(stream)), "sap_set_stream")
+    return h.value
+
+
+def sap_run(h: int, steps: int) -> None:
+    _check(_lib.sap_run(h, steps), "sap_run")
+
+
+def sap_run_levels(h: int, n_levels: int, group_size: int = 0) -> None:
+    _check(_lib.sap_run_levels(h, n_levels, group_size), "sap_run_levels")
+
+
+def sap_best(h: int, n_params: int):
+    fit, chain = C.c_uint32(), C.c_int32()
+    params = np.zeros(n_params, dtype=np.int8)
+    _check(_lib.sap_best(h, C.byref(fit), C.byref(chain), params.ctypes.data), "sap_best")
+    return fit.value, chain.value, params
+
+
+def sap_destroy(h: int) -> None:
+    _lib.sap_destroy(h)
+
+
+def sap_eval(h: int, params) -> np.ndarray:
+    x = _arr(params, np.int8)
+    x = x.reshape(-1, x.shape[-1])
+    out = np.zeros(x.shape[0], dtype=np.uint32)
+    _check(_lib.sap_eval(h, x.ctypes.data, x.shape[0], out.ctypes.data), "sap_eval")
+    return out
+
+
+def sap_simulate(prob, params) -> np.ndarray:
+    net, obs, keep = _marshal_paper(prob, need_ref=False)
+    x = _arr(params, np.int8)
+    out = np.zeros((prob.n_cond, prob.n_steps + 1, prob.n_nodes), dtype=np.uint8)
+    _check(_lib.sap_simulate(C.byref(net), C.byref(obs), x.ctypes.data, out.ctypes.data), "sap_simulate")
+    return out
+
+
+def sap_get_chain(h: int, chain: int, n_params: int):
+    cur = np.zeros(n_params, dtype=np.int8)
+    best = np.zeros(n_params, dtype=np.int8)
+    fc, fb = C.c_uint32(), C.c_uint32()
+    _check(_lib.sap_get_chain(h, chain, cur.ctypes.data, C.byref(fc), best.ctypes.data, C.byref(fb)), "sap_get_chain")
+    return cur, fc.value, best, fb.value
+
+
+def sap_get_fitness(h: int, n_chains: int):
+    cur = np.zeros(n_chains, dtype=np.uint32)
+    best = np.zeros(n_chains, dtype=np.uint32)
+    _check(_lib.sap_get_fitness(h, cur.ctypes.data, best.ctypes.data), "sap_get_fitness")
+    return cur, best
+
+
+def sap_set_trace(h: int, chains: Sequence[int], max_steps: int) -> None:
+    c = _arr(list(chains), np.int32)
+    _check(_lib.sap_set_trace(h, c.ctypes.data if c.size else None, int(c.size), max_steps), "sap_set_trace")
+
+
+def sap_get_trace(h: int, n_chains: int, max_steps: int) -> np.ndarray:
+    out = np.zeros((n_chains, max_steps), dtype=np.uint64)
+    _check(_lib.sap_get_trace(h, out.ctypes.data), "sap_get_trace")
+    return out
+
+
+def sap_get_level_stats(h: int, n_levels: int) -> dict:
+    out = np.zeros((n_levels, 4), dtype=np.uint64)
+    _check(_lib.sap_get_level_stats(h, out.ctypes.data), "sap_get_level_stats")
+    return {"steps": out[:, 0].astype(np.int64), "accepted": out[:, 1].astype(np.int64),
+            "accepted_worse": out[:, 2].astype(np.int64), "improved": out[:, 3].astype(np.int64)}
+
+
+def sap_get_info(h: int) -> dict:
+    info = np.zeros(12, dtype=np.int64)
+    _check(_lib.sap_get_info(h, info.ctypes.data), "sap_get_info")
+    keys = ("lanes_per_chain", "node_slots", "edge_slots", "threads_per_cta", "chains_per_cta", "smem_bytes", "grid",
+            "regs", "ctas_per_sm", "sm_count", "launches", "max_objective")
+    return dict(zip(keys, (int(v) for v in info)))
+
+
+def sap_jit_check(prob) -> dict:
+    """Host only: plan + NVRTC compile of the paper-model kernels for this network."""
+    net, obs, keep = _marshal_paper(prob, need_ref=getattr(prob, "ref", None) is not None)
+    info = np.zeros(4, dtype=np.int64)
+    log = C.create_string_buffer(16384)
+    _check(_lib.sap_jit_check(C.byref(net), C.byref(obs), info.ctypes.data, log, len(log)), "sap_jit_check")
+    return {"lanes_per_chain": int(info[0]), "node_slots": int(info[1]), "edge_slots": int(info[2]),
+            "cubin_bytes": int(info[3]), "log": log.value.decode(errors="replace")}

@@ -12,9 +12,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libternary_sa.so")
 SOURCES = ["sa_api.cu", "sa_kernels.cu", "sa_peak.cu", "sa_plan.cpp", "sa_dense_plan.cpp", "sa_jit.cpp", "sa_static_aot.cu",
-           "sa_dense_aot.cu"]
+           "sa_dense_aot.cu", "sap_api.cu", "sap_plan.cpp", "sap_aot.cu"]
 EMBED = {"sa_static_source.inc": ("sa_static_params.h", "sa_static_kernel.cu"),
-         "sa_dense_source.inc": ("sa_dense_params.h", "sa_dense_kernel.cu")}
+         "sa_dense_source.inc": ("sa_dense_params.h", "sa_dense_kernel.cu"),
+         "sap_source.inc": ("sap_params.h", "sap_kernel.cu")}
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-Wall", "--use_fast_math"]
 

@@ -11,62 +11,19 @@
 
 #include "../../include/ternary_sa.h"
 #include "sa_common.h"
+#include "sa_host.h"
 #include "sa_jit.h"
 #include "sa_kernels.h"
 #include "sa_plan.h"
 
 namespace {
 
-thread_local std::string g_err;
-sa_alloc_fn g_alloc = nullptr;
-sa_free_fn g_free = nullptr;
-
-int set_err(int code, const std::string& msg) {
-  g_err = msg;
-  return code;
-}
-
-int cuda_err(cudaError_t e, const char* what) {
-  return set_err(SA_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
-}
-
-#define TSA_CUDA(call)                                   \
-  do {                                                   \
-    cudaError_t e__ = (call);                            \
-    if (e__ != cudaSuccess) return cuda_err(e__, #call); \
-  } while (0)
-
-// Device buffers owned by a handle; released through the hooks they were allocated with.
-struct DevPool {
-  std::vector<void*> ptrs;
-  sa_free_fn release = nullptr;
-  bool hooked = false;
-  ~DevPool() { clear(); }
-  void clear() {
-    for (void* p : ptrs) {
-      if (!p) continue;
-      if (hooked) release(p); else cudaFree(p);
-    }
-    ptrs.clear();
-  }
-  void* alloc(size_t bytes, cudaStream_t st) {
-    if (bytes == 0) bytes = 16;
-    void* p = nullptr;
-    if (ptrs.empty()) { hooked = (g_alloc && g_free); release = g_free; }
-    if (hooked) p = g_alloc(bytes, (void*)st);
-    else if (cudaMalloc(&p, bytes) != cudaSuccess) { cudaGetLastError(); p = nullptr; }
-    if (p) ptrs.push_back(p);
-    return p;
-  }
-  template <typename T>
-  int upload(const std::vector<T>& v, const T** out, cudaStream_t st) {
-    T* d = (T*)alloc(v.size() * sizeof(T), st);
-    if (!d) return set_err(SA_ENOMEM, "device allocation failed");
-    if (!v.empty()) TSA_CUDA(cudaMemcpyAsync(d, v.data(), v.size() * sizeof(T), cudaMemcpyHostToDevice, st));
-    *out = d;
-    return SA_OK;
-  }
-};
+using tsa::cuda_err;
+using tsa::DevPool;
+using tsa::g_alloc;
+using tsa::g_err;
+using tsa::g_free;
+using tsa::set_err;
 
 int upload_problem(const tsa::Plan& pl, DevPool& pool, tsa::DevProblem* P, cudaStream_t st) {
   tsa::DevProblem& d = *P;

@@ -11,6 +11,8 @@
 #include "sa_dense_plan.h"
 #include "sa_plan.h"
 #include "sa_static_params.h"
+#include "sap_params.h"
+#include "sap_plan.h"
 
 namespace tsa {
 
@@ -58,5 +60,14 @@ bool dense_kernel_compile(const std::vector<std::string>& defines, std::string* 
 int dense_chains_per_cta(const DensePlan& dp, const StaticTuning& tune);
 const StaticKernel* dense_kernel_get(const Plan& plan, const DensePlan& dp, const StaticTuning& tune, std::string* why);
 int dense_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_dense::Params& params, std::string* why);
+
+// The paper-model kernels, sap_kernel.cu: one module with three entry points (tsp_run, tsp_eval, tsp_init).
+struct PaperKernels {
+  StaticKernel run, eval, init;
+};
+std::vector<std::string> paper_kernel_defines(const PaperPlan& plan, int warps_per_cta, int min_blocks);
+bool paper_kernel_compile(const std::vector<std::string>& defines, std::string* cubin, std::string* log);
+const PaperKernels* paper_kernels_get(const PaperPlan& plan, std::string* why);
+int paper_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_paper::Params& params, std::string* why);
 
 }  // namespace tsa

@@ -24,7 +24,7 @@ def B():
 def _declared_functions():
     text = open(os.path.join(ROOT, "include", "ternary_sa.h")).read()
     text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(sa_[a-z0-9_]+)\s*\(", text)) - {"sa_alloc_fn", "sa_free_fn"})
+    return sorted(set(re.findall(r"\b(sap?_[a-z0-9_]+)\s*\(", text)) - {"sa_alloc_fn", "sa_free_fn"})
 
 
 def test_library_exports_every_declared_symbol(B):
@@ -126,3 +126,70 @@ def test_execution_plan_is_valid_for_every_config(B, problems_cache):
     finally:
         del os.environ["TSA_NO_SPLIT"], os.environ["TSA_NO_BANKOPT"]
     assert naive["split_nodes"] == 0 and naive["edge_iterations"] > mtb["edge_iterations"]
+
+
+# ------------------------------------------------------------------ the paper model (sap_*)
+@pytest.fixture(scope="module")
+def paper_hpg():
+    from oracle import oracle_paper as OP
+    from paper_2506_19866_b200 import problems as PB
+    return PB.make_paper_problem("paper_hpg", OP.simulate_fn)
+
+
+def test_sap_create_validation(B, paper_hpg):
+    from paper_2506_19866_b200 import problems as PB
+    good = paper_hpg
+    sched = PB.paper_schedule(8, 4, 10, good.max_objective)
+
+    def bad(prob, sc, match, flags=0):
+        with pytest.raises(B.SaError) as ei:
+            B.sap_create(prob, sc, flags)
+        assert ei.value.code == B.SA_EINVAL and match in str(ei.value), str(ei.value)
+
+    p = copy.copy(good); p.edge_src = good.edge_src.copy(); p.edge_src[0] = p.edge_dst[0]
+    bad(p, sched, "self-loop")
+    p = copy.copy(good); p.edge_src = good.edge_src.copy(); p.edge_dst = good.edge_dst.copy()
+    p.edge_src[1], p.edge_dst[1] = p.edge_src[0], p.edge_dst[0]
+    bad(p, sched, "duplicate")
+    p = copy.copy(good); p.edge_dst = good.edge_dst.copy(); p.edge_dst[0] = good.n_nodes
+    bad(p, sched, "out of range")
+    p = copy.copy(good); p.fast = good.fast.copy(); p.fast[0] = 2
+    bad(p, sched, "fast")
+    p = copy.copy(good); p.init_state = good.init_state.copy(); p.init_state[0, 0] = 3
+    bad(p, sched, "initial state")
+    p = copy.copy(good); p.ref = good.ref.copy(); p.ref[0, 0, 0] = 9
+    bad(p, sched, "reference")
+    s = copy.copy(sched); s.n_chains = 0
+    bad(good, s, "schedule")
+    bad(good, sched, "flag", flags=64)
+    # with constraints on, a node without an in-edge admits no valid vector
+    p = copy.copy(good)
+    keep = good.edge_dst != good.edge_dst[0]
+    p.edge_src, p.edge_dst, p.n_edges = good.edge_src[keep], good.edge_dst[keep], int(keep.sum())
+    bad(p, sched, "in-edge", flags=B.SAP_CONSTRAINED)
+    B.sap_destroy(None)
+
+
+def test_paper_kernels_compile_for_every_shape(B, paper_hpg):
+    """Host only: the plan and the NVRTC build of the paper-model kernels (no GPU needed)."""
+    from oracle import oracle_paper as OP
+    from paper_2506_19866_b200 import problems as PB
+    info = B.sap_jit_check(paper_hpg)
+    assert (info["lanes_per_chain"], info["node_slots"]) == (8, 2) and info["cubin_bytes"] > 0, info["log"]
+    indeg = np.bincount(paper_hpg.edge_dst, minlength=9)
+    top = np.sort(indeg)[::-1]
+    assert info["edge_slots"] == int(top[0] + top[8])            # slot 0 holds the 8 largest in-degrees, slot 1 the rest
+    mtb = B.sap_jit_check(PB.make_paper_problem("paper_mtb", OP.simulate_fn))
+    assert (mtb["lanes_per_chain"], mtb["node_slots"]) == (32, 2) and mtb["cubin_bytes"] > 0, mtb["log"]
+
+
+def test_no_cpu_fallback_paper_model(B, paper_hpg):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    from paper_2506_19866_b200 import problems as PB
+    with pytest.raises(B.SaError) as ei:
+        B.sap_create(paper_hpg, PB.paper_schedule(8, 4, 10, 64), 0)
+    assert ei.value.code in (B.SA_ECUDA, B.SA_ENOMEM)
+    with pytest.raises(B.SaError):
+        B.sap_simulate(paper_hpg, paper_hpg.truth)
