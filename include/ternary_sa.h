@@ -72,7 +72,9 @@ typedef struct {
  * Validation (SA_EINVAL): counts > 0, endpoints in range, no self-loop / duplicate edge,
  * th_lo < th_hi, states in {0,1,2}, obs in {0,1,2,255}, obs_times strictly increasing in [1,T],
  * accumulator range: 128 + s - th_lo[q] and 128 + s - th_hi[q] - 1 in [0,255] for all |s| <=
- * 2*max_in_degree (in-degree <= 62 with thresholds in [-3,3]).  On failure *out = NULL. */
+ * 2*max_in_degree (in-degree <= 62 with thresholds in [-3,3]); kernel limits: n_pairs in [2,16],
+ * n_steps <= 127, n_obs <= 127, E < 2^24, state entries x words per entry x 4 <= 65535 bytes (about
+ * 16 000 nodes at K <= 4, 4 000 at K <= 16).  On failure *out = NULL. */
 int sa_create(const sa_network *net, const sa_observations *obs, const sa_schedule *sched, sa_handle **out);
 
 /* Advance every chain by `steps` SA steps (Table 1 inner loop :130-149; SURVEY.md
@@ -152,7 +154,16 @@ int sa_get_dense_info(sa_handle *h, int64_t info[8]);
  * problem at hand by NVRTC at the first sa_run.  Else the generic one.  GENERIC: the ahead-of-time
  * compiled table-driven kernels.  STATIC / DENSE: that family only; sa_run fails with SA_EINVAL /
  * SA_ECUDA (reason in sa_last_error) instead of falling back.  All families produce identical
- * results.  Environment override: TSA_KERNEL=generic|static|dense. */
+ * results.
+ *
+ * Environment.  Always read: TSA_KERNEL=generic|static|dense overrides sa_select_kernel (also cta|warp:
+ * the generic family with one CTA / one warp per chain); TSA_NVRTC_LIB=<path> names the libnvrtc to load.
+ * Read ONLY when TSA_TUNING=1 (measurements and the parity tests, which show that none of them changes
+ * a result): TSA_TEAM_WARPS, TSA_TEAM_MIN, TSA_CPB, TSA_NO_SPLIT, TSA_NO_BANKOPT,
+ * TSA_NO_TIERS, TSA_MAX_SLOTS (generic / static launch shape and host schedule); TSA_JIT_REGS,
+ * TSA_JIT_BATCH, TSA_JIT_TUNROLL (static kernel); TSA_DENSE_BLOCKS, TSA_DENSE_PH, TSA_DENSE_CPB,
+ * TSA_DENSE_SWZ, TSA_DENSE_SP, TSA_DENSE_W, TSA_DENSE_REDERIVE, TSA_DENSE_TUNROLL, TSA_DENSE_EARLY_OBS,
+ * TSA_DENSE_NO_BALANCE (dense kernel); TSA_PAPER_LPC, TSA_PAPER_WPB, TSA_PAPER_BLOCKS (paper model). */
 #define SA_KERNEL_AUTO    0
 #define SA_KERNEL_GENERIC 1
 #define SA_KERNEL_STATIC  2
@@ -277,6 +288,11 @@ int sa_set_allocator(sa_alloc_fn alloc, sa_free_fn release);
  * in warp-instructions per second (whole GPU); out[4] = SM count, out[5] = SM clock in Hz as
  * observed through clock64 over the run.  (SURVEY.md §8(d) "Which roofline".) */
 int sa_int32_peak(double out[6]);
+
+/* Second ceiling of the dense kernel, measured: issue rates of the legacy int8 tensor path on the current
+ * device, in MMA instructions per second (whole GPU): out[0] = mma.sync m16n8k32 s8 (SASS IMMA.16832.S8),
+ * out[1] = mma.sp m16n8k64 s8 (IMMA.SP.16864.S8), out[2] = SM count, out[3] = SM clock in Hz observed. */
+int sa_imma_peak(double out[4]);
 
 const char *sa_last_error(void);
 

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libternary_sa.so")
 SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
-           "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_last_error", "sa_plan_info",
+           "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_imma_peak", "sa_last_error", "sa_plan_info",
            "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info",
            "sap_create", "sap_run", "sap_run_levels", "sap_best", "sap_destroy", "sap_eval", "sap_simulate",
            "sap_get_chain", "sap_get_fitness", "sap_set_trace", "sap_get_trace", "sap_get_level_stats", "sap_get_info",
@@ -79,6 +79,7 @@ _lib.sa_plan_info.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c
 _lib.sa_set_stream.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_set_allocator.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_int32_peak.argtypes = [C.c_void_p]
+_lib.sa_imma_peak.argtypes = [C.c_void_p]
 _lib.sa_select_kernel.argtypes = [C.c_void_p, C.c_int]
 _lib.sa_jit_check.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c_int32, C.c_void_p, C.c_char_p, C.c_size_t]
 
@@ -302,6 +303,12 @@ def sa_int32_peak() -> dict:
     out = np.zeros(6, dtype=np.float64)
     _check(_lib.sa_int32_peak(out.ctypes.data), "sa_int32_peak")
     return {"iadd3": out[0], "lop3": out[1], "imad": out[2], "mixed": out[3], "sm_count": int(out[4]), "sm_hz": out[5]}
+
+
+def sa_imma_peak() -> dict:
+    out = np.zeros(4, dtype=np.float64)
+    _check(_lib.sa_imma_peak(out.ctypes.data), "sa_imma_peak")
+    return {"imma_16832": out[0], "imma_sp_16864": out[1], "sm_count": int(out[2]), "sm_hz": out[3]}
 
 
 def sa_last_error() -> str:

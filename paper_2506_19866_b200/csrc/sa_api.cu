@@ -9,6 +9,7 @@
 #include <string>
 #include <vector>
 
+#include "sa_tuning.h"
 #include "../../include/ternary_sa.h"
 #include "sa_common.h"
 #include "sa_host.h"
@@ -59,7 +60,7 @@ int upload_problem(const tsa::Plan& pl, DevPool& pool, tsa::DevProblem* P, cudaS
 }
 
 int pick_threads(const tsa::DevProblem& P, int64_t n_ctas, int sm_count) {
-  if (const char* env = std::getenv("TSA_TEAM_WARPS")) {
+  if (const char* env = tsa::tune_env("TSA_TEAM_WARPS")) {
     int w = std::atoi(env);
     if (w >= 1 && w <= 32) return 32 * w;
   }
@@ -81,7 +82,7 @@ int pick_warp_cpb(const tsa::DevProblem& P, int64_t R, int sm_count) {
     if (std::string(env) == "cta") return 0;
     if (std::string(env) == "warp" && P.n_pass <= 32) {
       int cpb = 8;
-      if (const char* c = std::getenv("TSA_CPB")) cpb = std::max(1, std::min(8, std::atoi(c)));
+      if (const char* c = tsa::tune_env("TSA_CPB")) cpb = std::max(1, std::min(8, std::atoi(c)));
       return tsa::warp_kernel_smem(P, cpb) <= 227 * 1024 ? cpb : 0;
     }
   }
@@ -134,6 +135,7 @@ struct sa_handle {
   const tsa::StaticKernel* dk = nullptr;
   bool dk_tried = false;
   uint32_t* d_flags = nullptr;      // [R] hand-over flags of the balanced launch
+  uint32_t* d_err = nullptr;        // [1] raised by a kernel whose hand-over wait gave up
   unsigned long long* d_win = nullptr;   // [R] winners of the level synchronisation (sa_run_levels)
   int64_t last_slot_steps = 0;
   std::string dense_why;
@@ -160,7 +162,7 @@ bool use_dense(sa_handle* h) {
   if (!h->dk_tried) {
     h->dk_tried = true;
     tsa::StaticTuning tune = tsa::StaticTuning::from_env();
-    if (!std::getenv("TSA_DENSE_BLOCKS")) {
+    if (!tsa::tune_env("TSA_DENSE_BLOCKS")) {
       // fewer chains than slots: do not squeeze the registers for an occupancy the grid cannot reach
       const int per_sm = (int)((h->C.R + h->sm_count - 1) / std::max(h->sm_count, 1));
       tune.dense_blocks = std::max(1, std::min(h->dplan.sparse ? 16 : 12, per_sm));
@@ -187,6 +189,7 @@ tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
   q.trace_row = h->Tr.row_of_chain; q.trace_rec = (tsa_dense::u64*)h->Tr.records;
   q.trace_max = h->Tr.max_steps; q.trace_g0 = h->Tr.g_start;
   q.g0 = h->g; q.steps = steps;
+  q.err = h->d_err;
   return q;
 }
 
@@ -224,7 +227,7 @@ tsa_static::Params static_params(const sa_handle* h, int64_t steps) {
 
 tsa::PlanOptions plan_options(int64_t n_chains, int sm_count) {
   tsa::PlanOptions o = tsa::PlanOptions::from_env();
-  if (!std::getenv("TSA_TEAM_MIN")) {
+  if (!tsa::tune_env("TSA_TEAM_MIN")) {
     // few chains: spread each over more warps so that an SM still sees ~16 resident warps
     const int64_t want = (16LL * sm_count + n_chains - 1) / std::max<int64_t>(n_chains, 1);
     o.min_team_warps = (int)std::max<int64_t>(1, std::min<int64_t>(32, want));
@@ -294,7 +297,9 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->dplan.wloc, &h->d_dwloc, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.thloc, &h->d_dthloc, st))) return rc;
     h->d_flags = (uint32_t*)h->pool.alloc((size_t)sched->n_chains * 4, st);
-    if (!h->d_flags) return set_err(SA_ENOMEM, "device allocation failed (flags)");
+    h->d_err = (uint32_t*)h->pool.alloc(4, st);
+    if (!h->d_flags || !h->d_err) return set_err(SA_ENOMEM, "device allocation failed (flags)");
+    TSA_CUDA(cudaMemsetAsync(h->d_err, 0, 4, st));
   }
 
   const int R = sched->n_chains;
@@ -355,7 +360,7 @@ int sa_run(sa_handle* h, int64_t steps) {
     // (DESIGN.md §6 "balanced slots") instead of running ceil(R / slots) uneven waves.
     const int64_t slots = (int64_t)h->dk->blocks_per_sm * h->sm_count;
     h->last_slot_steps = 0;
-    if (h->dk->chains_per_cta == 1 && slots > 0 && h->C.R > slots && !std::getenv("TSA_DENSE_NO_BALANCE")) {
+    if (h->dk->chains_per_cta == 1 && slots > 0 && h->C.R > slots && !tsa::tune_env("TSA_DENSE_NO_BALANCE")) {
       const int64_t total = (int64_t)h->C.R * steps;
       q.slot_steps = std::max<int64_t>((total + slots - 1) / slots, steps);
       q.flags = h->d_flags;
@@ -363,7 +368,19 @@ int sa_run(sa_handle* h, int64_t steps) {
       grid = (unsigned)((total + q.slot_steps - 1) / q.slot_steps);
       h->last_slot_steps = q.slot_steps;
     }
-    if (tsa::dense_kernel_launch(h->dk, grid, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
+    // A slot that holds the tail of a chain waits for the slot that holds its head, so every slot must
+    // be resident at once: the balanced launch is cooperative.  If the device cannot take the whole
+    // grid right now (another context holds SMs), fall back to the plain launch, one chain per CTA.
+    bool launched = false;
+    if (q.slot_steps > 0) {
+      launched = tsa::dense_kernel_launch(h->dk, grid, (void*)h->stream, q, &why, true) == 0;
+      if (!launched) {
+        q.slot_steps = 0; q.flags = nullptr;
+        h->last_slot_steps = 0;
+        grid = (unsigned)h->C.R;
+      }
+    }
+    if (!launched && tsa::dense_kernel_launch(h->dk, grid, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
     ++h->launches;
     h->g += (uint64_t)steps;
     return SA_OK;
@@ -411,13 +428,23 @@ int sa_run_levels(sa_handle* h, int64_t n_levels, int32_t group_size) {
   return SA_OK;
 }
 
+// after a stream synchronisation: did a kernel of this handle give up a hand-over wait?
+static int check_device_error(sa_handle* h) {
+  if (!h->d_err) return SA_OK;
+  uint32_t e = 0;
+  TSA_CUDA(cudaMemcpyAsync(&e, h->d_err, 4, cudaMemcpyDeviceToHost, h->stream));
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  if (e) return set_err(SA_ECUDA, "a balanced-slot hand-over wait timed out; the chains of this handle are invalid");
+  return SA_OK;
+}
+
 int sa_get_fitness(sa_handle* h, uint32_t* cur_fit, uint32_t* best_fit) {
   if (!h) return set_err(SA_EINVAL, "null handle");
   const size_t bytes = (size_t)h->C.R * 4;
   if (cur_fit) TSA_CUDA(cudaMemcpyAsync(cur_fit, h->C.fit_cur, bytes, cudaMemcpyDeviceToHost, h->stream));
   if (best_fit) TSA_CUDA(cudaMemcpyAsync(best_fit, h->C.fit_best, bytes, cudaMemcpyDeviceToHost, h->stream));
   TSA_CUDA(cudaStreamSynchronize(h->stream));
-  return SA_OK;
+  return check_device_error(h);
 }
 
 int sa_get_chain(sa_handle* h, int32_t chain, int8_t* cur, uint32_t* cur_fit, int8_t* best, uint32_t* best_fit) {
@@ -441,7 +468,7 @@ int sa_get_chain(sa_handle* h, int32_t chain, int8_t* cur, uint32_t* cur_fit, in
   if (cur_fit) TSA_CUDA(cudaMemcpyAsync(cur_fit, h->C.fit_cur + chain, 4, cudaMemcpyDeviceToHost, st));
   if (best_fit) TSA_CUDA(cudaMemcpyAsync(best_fit, h->C.fit_best + chain, 4, cudaMemcpyDeviceToHost, st));
   TSA_CUDA(cudaStreamSynchronize(st));
-  return SA_OK;
+  return check_device_error(h);
 }
 
 int sa_best(sa_handle* h, uint32_t* fitness, int32_t* chain, int8_t* params) {

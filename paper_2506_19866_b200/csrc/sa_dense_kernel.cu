@@ -96,10 +96,6 @@ __device__ __forceinline__ u32 sign_mask(u32 x) {
 
 // D (16 x 8, s32) += A (16 x 32, s8, row) * B (32 x 8, s8, col)
 __device__ __forceinline__ void imma(int (&c)[4], const u32* a, u32 b0, u32 b1) {
-#ifdef TSD_PROBE_NO_IMMA      // timing probe only (wrong results): what the time step costs without the tensor pipe
-  c[0] += (int)(a[0] ^ b0); c[1] += (int)(a[1] ^ b1); c[2] += (int)a[2]; c[3] += (int)a[3];
-  return;
-#endif
   asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
@@ -400,7 +396,13 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
 
   if (s0 > 0) {                              // the head of this chain is another slot's first piece
     if (tix == 0) {
-      while (*(volatile u32*)(p.flags + chain) == 0u) __nanosleep(200);
+      // the launch is cooperative (every slot is resident) and a head piece never waits, so this wait ends;
+      // it is bounded all the same (about 2^26 x 200 ns) and reports instead of hanging the device
+      u32 spins = 0u;
+      while (*(volatile u32*)(p.flags + chain) == 0u) {
+        __nanosleep(200);
+        if (++spins > (1u << 26)) { atomicExch(p.err, 1u); break; }
+      }
       __threadfence();
     }
     team_sync();

@@ -54,6 +54,7 @@ struct Params {
   // of R*steps; flags[chain] != 0 once the head piece of a straddling chain is back in HBM
   i64 slot_steps;
   u32* flags;             // [R], zeroed by the host before the launch
+  u32* err;               // [1] set to 1 if a hand-over wait gave up (the launch's results are then invalid)
 };
 
 }  // namespace tsa_dense

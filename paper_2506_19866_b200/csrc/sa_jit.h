@@ -59,7 +59,9 @@ bool dense_kernel_compile(const std::vector<std::string>& defines, std::string* 
 // chains per CTA the kernel will be built for (1 unless the plan has one-warp chains)
 int dense_chains_per_cta(const DensePlan& dp, const StaticTuning& tune);
 const StaticKernel* dense_kernel_get(const Plan& plan, const DensePlan& dp, const StaticTuning& tune, std::string* why);
-int dense_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_dense::Params& params, std::string* why);
+// cooperative = true: cuLaunchCooperativeKernel (every CTA of the grid resident at once, or the launch fails)
+int dense_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_dense::Params& params, std::string* why,
+                        bool cooperative = false);
 
 // The paper-model kernels, sap_kernel.cu: one module with three entry points (tsp_run, tsp_eval, tsp_init).
 struct PaperKernels {

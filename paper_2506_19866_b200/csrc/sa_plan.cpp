@@ -1,3 +1,4 @@
+#include "sa_tuning.h"
 #include "sa_plan.h"
 
 #include "sa_common.h"
@@ -273,11 +274,11 @@ void colour_group(const std::vector<std::vector<int>>& lane_banks, int nb, int c
 
 PlanOptions PlanOptions::from_env() {
   PlanOptions o;
-  if (const char* e = std::getenv("TSA_NO_SPLIT")) o.split_rows = !(e[0] == '1');
-  if (const char* e = std::getenv("TSA_NO_BANKOPT")) o.bank_opt = !(e[0] == '1');
-  if (const char* e = std::getenv("TSA_NO_TIERS")) o.tiers = !(e[0] == '1');
-  if (const char* e = std::getenv("TSA_TEAM_MIN")) o.min_team_warps = std::max(1, std::atoi(e));
-  if (const char* e = std::getenv("TSA_MAX_SLOTS")) o.max_lane_slots = std::max(0, std::atoi(e));
+  if (const char* e = tsa::tune_env("TSA_NO_SPLIT")) o.split_rows = !(e[0] == '1');
+  if (const char* e = tsa::tune_env("TSA_NO_BANKOPT")) o.bank_opt = !(e[0] == '1');
+  if (const char* e = tsa::tune_env("TSA_NO_TIERS")) o.tiers = !(e[0] == '1');
+  if (const char* e = tsa::tune_env("TSA_TEAM_MIN")) o.min_team_warps = std::max(1, std::atoi(e));
+  if (const char* e = tsa::tune_env("TSA_MAX_SLOTS")) o.max_lane_slots = std::max(0, std::atoi(e));
   return o;
 }
 

@@ -1,3 +1,4 @@
+#include "sa_tuning.h"
 #include "sap_plan.h"
 
 #include <algorithm>
@@ -57,7 +58,7 @@ int build_paper_plan(const sap_network* net, const sap_observations* obs, bool n
 
   // lanes per chain, node slots; nodes sorted by in-degree so that a node slot holds nodes of similar degree
   pl.LPC = N <= 16 ? 8 : N <= 32 ? 16 : 32;
-  if (const char* e = std::getenv("TSA_PAPER_LPC")) {
+  if (const char* e = tsa::tune_env("TSA_PAPER_LPC")) {
     const int v = std::atoi(e);
     if ((v == 8 || v == 16 || v == 32) && 8 * v >= N) pl.LPC = v;
   }

@@ -4,6 +4,9 @@ import sys
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+# the library reads its launch-geometry knobs (TSA_DENSE_*, TSA_TEAM_*, ... see include/ternary_sa.h) only under this
+# switch; the parity tests use them to show that no setting changes a result
+os.environ["TSA_TUNING"] = "1"
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 

@@ -70,3 +70,39 @@ def test_reference_arm_prints_on_rank0_only():
     assert len(lines) == 1
     d = json.loads(lines[0])
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["cpu_baseline"]["kind"] == "oracle"
+
+
+def test_gpus_flag_without_torchrun():
+    """`python bench.py --gpus 2` as the driver runs it, with no torchrun environment: the reference arm
+    runs in this one process and reports n_gpus = 2; our arm starts two ranks itself, and on a box
+    without two CUDA devices each of them fails loudly instead of measuring one GPU as if it were two."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1",
+                          "--warmup", "0", "--workload", "paper_hpg"], capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and "paper model" in d["config"]["workload"]
+    import torch
+    if torch.cuda.is_available() and torch.cuda.device_count() >= 2:
+        return
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0",
+                          "--workload", "tiny", "--no-extra"], capture_output=True, text=True, timeout=600, env=env, cwd=ROOT)
+    assert out.returncode != 0
+    assert not [l for l in out.stdout.splitlines() if l.startswith("{")]          # no bench line from a run that cannot be N = 2
+    assert "CUDA device" in out.stderr or "CUDA devices" in out.stderr
+
+
+def test_instruction_counts_file_names_existing_captures():
+    """profiles/inst_counts.json (the per-kernel instruction counts bench.py turns into the issue-slot
+    fraction) cites capture summaries that exist under profiles/."""
+    with open(os.path.join(ROOT, "profiles", "inst_counts.json")) as f:
+        counts = json.load(f)
+    assert "mtb" in counts
+    for name, c in counts.items():
+        if name.startswith("_"):
+            continue
+        assert c["warp_inst_per_chain_step"] > 0 and c["kernel"]
+        cited = c["source"].split()[0]
+        assert os.path.exists(os.path.join(ROOT, cited)), cited
