@@ -99,15 +99,30 @@ __device__ __forceinline__ void team_sync() {
   if (W == 1) __syncwarp(); else __syncthreads();
 }
 
+// Debug build (-DTSA_BOUNDS=1, set by TSA_BOUNDS_CHECK=1 under TSA_TUNING=1): every shared-memory access made
+// through the helpers below is checked against the CTA's dynamic shared-memory window and its own
+// alignment, and traps if it falls outside (compute-sanitizer is not available on the GPU pool).
+#ifdef TSA_BOUNDS
+__device__ __forceinline__ void smem_check(u32 a, u32 bytes) {
+  u32 total, base;
+  asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(total));
+  { extern __shared__ __align__(16) unsigned char tsa_smem_window[]; base = (u32)__cvta_generic_to_shared(tsa_smem_window); }
+  if (a < base || a + bytes > base + total || (a & (bytes - 1u)) != 0u) __trap();
+}
+#else
+__device__ __forceinline__ void smem_check(u32, u32) {}
+#endif
 // shared memory through 32-bit shared-window addresses
-__device__ __forceinline__ void lds(u32 a, u32 (&s)[1]) { asm volatile("ld.shared.u32 %0, [%1];" : "=r"(s[0]) : "r"(a) : "memory"); }
-__device__ __forceinline__ void lds(u32 a, u32 (&s)[2]) { asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(s[0]), "=r"(s[1]) : "r"(a) : "memory"); }
+__device__ __forceinline__ void lds(u32 a, u32 (&s)[1]) { smem_check(a, 4); asm volatile("ld.shared.u32 %0, [%1];" : "=r"(s[0]) : "r"(a) : "memory"); }
+__device__ __forceinline__ void lds(u32 a, u32 (&s)[2]) { smem_check(a, 8); asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(s[0]), "=r"(s[1]) : "r"(a) : "memory"); }
 __device__ __forceinline__ void lds(u32 a, u32 (&s)[4]) {
+  smem_check(a, 16);
   asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(s[0]), "=r"(s[1]), "=r"(s[2]), "=r"(s[3]) : "r"(a) : "memory");
 }
-__device__ __forceinline__ void sts(u32 a, const u32 (&s)[1]) { asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(s[0]) : "memory"); }
-__device__ __forceinline__ void sts(u32 a, const u32 (&s)[2]) { asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(a), "r"(s[0]), "r"(s[1]) : "memory"); }
+__device__ __forceinline__ void sts(u32 a, const u32 (&s)[1]) { smem_check(a, 4); asm volatile("st.shared.u32 [%0], %1;" ::"r"(a), "r"(s[0]) : "memory"); }
+__device__ __forceinline__ void sts(u32 a, const u32 (&s)[2]) { smem_check(a, 8); asm volatile("st.shared.v2.u32 [%0], {%1, %2};" ::"r"(a), "r"(s[0]), "r"(s[1]) : "memory"); }
 __device__ __forceinline__ void sts(u32 a, const u32 (&s)[4]) {
+  smem_check(a, 16);
   asm volatile("st.shared.v4.u32 [%0], {%1, %2, %3, %4};" ::"r"(a), "r"(s[0]), "r"(s[1]), "r"(s[2]), "r"(s[3]) : "memory");
 }
 

@@ -45,7 +45,7 @@ int upload_plan(const tsa::PaperPlan& pl, DevPool& pool, tsa_paper::Params* q, c
   if ((rc = pool.upload(pl.slot_edge, &q->slot_edge, st))) return rc;
   if ((rc = pool.upload(pl.pos_node, &q->pos_node, st))) return rc;
   if ((rc = pool.upload(pl.init_lane, &q->init_lane, st))) return rc;
-  if ((rc = pool.upload(pl.ref_lane, &q->ref_lane, st))) return rc;
+  if ((rc = pool.upload(pl.cost_lane, &q->cost_lane, st))) return rc;
   if ((rc = pool.upload(pl.fast, &q->fast, st))) return rc;
   if ((rc = pool.upload(pl.in_ptr, &q->in_ptr, st))) return rc;
   if ((rc = pool.upload(pl.in_edge, &q->in_edge, st))) return rc;
@@ -105,7 +105,7 @@ int sap_create(const sap_network* net, const sap_observations* obs, const sa_sch
   int dev = 0;
   cudaError_t dev_err = cudaGetDevice(&dev);
   if (dev_err == cudaSuccess) dev_err = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
-  int rc = tsa::build_paper_plan(net, obs, true, (flags & SAP_CONSTRAINED) != 0, &h->plan, &err);
+  int rc = tsa::build_paper_plan(net, obs, true, (flags & SAP_CONSTRAINED) != 0, sched->n_chains, h->sm_count, &h->plan, &err);
   if (rc != SA_OK) return set_err(rc, err);          // argument errors first, so validation works without a GPU
   if (dev_err != cudaSuccess) return cuda_err(dev_err, "cudaGetDevice");
   h->flags = flags;
@@ -267,7 +267,7 @@ int sap_simulate(const sap_network* net, const sap_observations* obs, const int8
   if (!net || !obs || !params || !states) return set_err(SA_EINVAL, "null argument");
   tsa::PaperPlan pl;
   std::string err;
-  int rc = tsa::build_paper_plan(net, obs, false, false, &pl, &err);
+  int rc = tsa::build_paper_plan(net, obs, false, false, 0, 148, &pl, &err);
   if (rc != SA_OK) return set_err(rc, err);
   if (!tsa::paper_params_valid(pl, params, 1)) return set_err(SA_EINVAL, "parameter value out of range");
   std::string why;
@@ -352,7 +352,7 @@ int sap_jit_check(const sap_network* net, const sap_observations* obs, int64_t i
   if (log && log_bytes) log[0] = 0;
   tsa::PaperPlan pl;
   std::string err;
-  const int rc = tsa::build_paper_plan(net, obs, obs->ref != nullptr, false, &pl, &err);
+  const int rc = tsa::build_paper_plan(net, obs, obs->ref != nullptr, false, 0, 148, &pl, &err);
   if (rc != SA_OK) return set_err(rc, err);
   info[0] = pl.LPC; info[1] = pl.NS; info[2] = pl.ES;
   std::string cubin, clog;

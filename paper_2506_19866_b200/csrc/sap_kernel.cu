@@ -6,9 +6,10 @@
 // node slot: the host sorts the nodes by in-degree so that slot n holds nodes of similar degree).  The
 // chain never leaves the chip during a launch:
 //   * per edge slot the lane keeps, in a register, a three-entry table of what the edge contributes to
-//     its target's image for source state 0 / 1 / 2:  4 + (s // t) * w * p  in bytes 0 / 1 / 2
-//     (PAPER.md:66-68); the source publishes its state as the 16-bit PRMT selector 0x4440 | s in a
-//     128-byte double-buffered shared array, so one edge costs LDS.U16 + PRMT + IADD;
+//     its target's image for source state 0 / 1 / 2:  4 + (s // t) * w * p  in bytes 1 / 2 / 3 (byte 0 = 0)
+//     (PAPER.md:66-68); the source publishes its state as the one-byte PRMT selector 0x41 + s in a
+//     double-buffered shared array of at most 128 bytes per warp (no bank conflicts), so one edge costs
+//     LDS.U8 + PRMT + IADD;
 //   * per node slot: clip the image to [0,2], eligibility from the memory count, priority = u x age,
 //     REDUX.MAX over the chain's lanes, bounded move, score against the
 //     reference with the gradient weight, publish the new state;
@@ -38,13 +39,15 @@ constexpr int LPC = TSP_LPC, NS = TSP_NS, G = 32 / LPC, WPB = TSP_WPB;
 constexpr int kESL[NS] = {TSP_ESL};                       // edge slots of node slot n
 __host__ __device__ constexpr int es_off(int n) { int s = 0; for (int i = 0; i < n; ++i) s += kESL[i]; return s; }
 constexpr int ES = es_off(NS);
+constexpr int NSP = NS <= 1 ? 1 : NS <= 2 ? 2 : NS <= 4 ? 4 : 8;   // node slots padded to a vector load
 constexpr int NPOS = NS * LPC;                            // node positions of a chain (>= N; the rest is padding)
-constexpr int STATE_B = NPOS * 2;                         // one state buffer of one chain: a 16-bit selector per position
+constexpr int STATE_B = NPOS;                             // one state buffer of one chain: a one-byte selector per position
 constexpr int BUF_B = G * STATE_B;                        // one state buffer of a warp's chains
 constexpr int NCPAD = (N + 3) / 4 * 4;
 constexpr int CHAIN_B = (NPPAD + 3 * NCPAD + 8 * 4 + 15) / 16 * 16;   // canonical vector, 3 counter rows, control words
 constexpr int WARP_B = (2 * BUF_B + 15) / 16 * 16 + G * CHAIN_B;
-constexpr u32 kEmptyLut = 0x00040404u;                    // an empty edge slot contributes 4 (= 0 after the bias) for every state
+constexpr u32 kEmptyLut = 0x04040400u;                    // an empty edge slot contributes 4 (= 0 after the bias) for every state
+constexpr u32 kSel0 = 0x41u;                              // selector of state s = kSel0 + s: byte s+1 of the table, then zeros
 static_assert(LPC == 8 || LPC == 16 || LPC == 32, "lanes per chain");
 static_assert(NS >= 1 && NS <= 8 && NPOS >= N, "node slots");
 static_assert(N <= 256 && ES <= 256, "ploc fields are 8 bits wide");
@@ -61,8 +64,28 @@ __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u3
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-__device__ __forceinline__ u32 lds_u16(u32 a) { u32 v; asm volatile("ld.shared.u16 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v; }
-__device__ __forceinline__ void sts_u16(u32 a, u32 v) { asm volatile("st.shared.u16 [%0], %1;" ::"r"(a), "h"((unsigned short)v) : "memory"); }
+// Debug build (-DTSA_BOUNDS=1, set by TSA_BOUNDS_CHECK=1 under TSA_TUNING=1): every shared-memory access made
+// through the helpers below is checked against the CTA's dynamic shared-memory window and its own
+// alignment, and traps if it falls outside (compute-sanitizer is not available on the GPU pool).
+#ifdef TSA_BOUNDS
+__device__ __forceinline__ void smem_check(u32 a, u32 bytes) {
+  u32 total, base;
+  asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(total));
+  { extern __shared__ __align__(16) unsigned char tsa_smem_window[]; base = (u32)__cvta_generic_to_shared(tsa_smem_window); }
+  if (a < base || a + bytes > base + total || (a & (bytes - 1u)) != 0u) __trap();
+}
+#else
+__device__ __forceinline__ void smem_check(u32, u32) {}
+#endif
+// shared memory through 32-bit shared-window addresses with a compile-time byte offset (which state buffer)
+template <int OFF>
+__device__ __forceinline__ u32 lds_u8(u32 a) { u32 v; smem_check(a + OFF, 1); asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(a), "n"(OFF) : "memory"); return v; }
+template <int OFF>
+__device__ __forceinline__ void sts_u8(u32 a, u32 v) { smem_check(a + OFF, 1); asm volatile("st.shared.u8 [%0+%1], %2;" ::"r"(a), "n"(OFF), "r"(v) : "memory"); }
+// byte look-up: result byte 0 = byte (sel & 7) of {table, 0}, byte 1 = byte 4 (zero), bytes 2-3 = byte 0 of the
+// table (kept zero).  Every selector here is 0x41 + state: no nibble has its replicate-sign bit set (the
+// __byte_perm intrinsic would spend an instruction masking them)
+__device__ __forceinline__ u32 prmt(u32 table, u32 sel) { u32 r; asm("prmt.b32 %0, %1, %2, %3;" : "=r"(r) : "r"(table), "r"(0u), "r"(sel)); return r; }
 
 // reductions over the LPC lanes of a chain (aligned lane groups of a full warp)
 __device__ __forceinline__ u32 group_max(u32 v) {
@@ -89,19 +112,20 @@ __device__ __forceinline__ int dom_size(int cls, bool fast) { return (cls == kT 
 __device__ __forceinline__ int dom_base(int cls, bool fast) { return cls == kP ? -1 : (cls == kT || cls == kD) ? 1 : cls == kU ? (fast ? 10 : 1) : 0; }
 __device__ __forceinline__ int class_of(int q) { return q < E ? kW : q < 2 * E ? kP : q < 3 * E ? kT : q < 3 * E + N ? kU : q < 3 * E + 2 * N ? kM : kD; }
 
-// contribution table of an edge: byte s = 4 + (s // t) * w * p  (floor division, reading 16)
+// contribution table of an edge: byte s+1 = 4 + (s // t) * w * p, byte 0 = 0  (floor division, reading 16)
 __device__ __forceinline__ u32 make_lut(int w, int p, int t) {
   const int c = w * p;
   const int v1 = t == 1 ? c : 0, v2 = t == 1 ? 2 * c : c;
-  return 4u | ((u32)(v1 + 4) << 8) | ((u32)(v2 + 4) << 16);
+  return (4u << 8) | ((u32)(v1 + 4) << 16) | ((u32)(v2 + 4) << 24);
 }
-__device__ __forceinline__ u32 make_nb(int u, int m, int d) { return (u32)u | ((u32)m << 4) | ((u32)d << 6); }
 
 // What a lane keeps in registers for its chain.
 struct Lane {
   u32 lut[ES];     // contribution table of each edge slot
   u32 addr[ES];    // shared address of the source's selector (state buffer 0)
-  u32 nb[NS];      // node slot: u | m << 4 | d << 6
+  u32 u[NS];       // node slot: speed u_i ...
+  u32 m[NS];       // ... memory m_i ...
+  int d[NS];       // ... step size d_i
   u32 self[NS];    // shared address of this lane's own selectors (state buffer 0)
   int node[NS];    // node id or -1
 };
@@ -118,38 +142,73 @@ __device__ __forceinline__ void build_lane(const Params& p, const i8* canon, u32
   for (int n = 0; n < NS; ++n) {
     const int i = __ldg(p.pos_node + n * LPC + lig);
     L.node[n] = i;
-    L.nb[n] = i < 0 ? make_nb(1, 0, 1) : make_nb(canon[3 * E + i], canon[3 * E + N + i], canon[3 * E + 2 * N + i]);
-    L.self[n] = sstate + (u32)(2 * (n * LPC + lig));
+    L.u[n] = i < 0 ? 1u : (u32)canon[3 * E + i];
+    L.m[n] = i < 0 ? 0u : (u32)canon[3 * E + N + i];
+    L.d[n] = i < 0 ? 1 : (int)canon[3 * E + 2 * N + i];
+    L.self[n] = sstate + (u32)(n * LPC + lig);
   }
 }
 
 // First half of a transition, node slot NI (a template so that the slot's edge-slot count is a constant
-// expression): the image from the published states of t-1, eligibility and priority.
-template <int NI>
+// expression), reading state buffer RB: the image from the published states of t-1, eligibility, priority.
+template <int NI, int RB>
 struct Images {
-  static __device__ __forceinline__ void run(const Lane& L, u32 rb, u32 t, const u32 (&s)[NS], const u32 (&last)[NS],
-                                             const u32 (&cnt)[NS], u32 (&tg)[NS], u32 (&pr)[NS], u32& top) {
+  static __device__ __forceinline__ void run(const Lane& L, u32 t, const u32 (&s)[NS], const u32 (&last)[NS], const u32 (&cnt)[NS],
+                                             u32 (&tg)[NS], u32 (&pr)[NS], u32& top) {
     constexpr int EO = es_off(NI), EN = kESL[NI];
     u32 acc = 0u;
 #pragma unroll
-    for (int j = 0; j < EN; ++j) {
-      const u32 sel = lds_u16(L.addr[EO + j] + rb);
-      acc += __byte_perm(L.lut[EO + j], 0u, sel);                       // 4 + (s_j // t_ji) * w_ji * p_ji
-    }
+    for (int j = 0; j < EN; ++j) acc += prmt(L.lut[EO + j], lds_u8<RB * BUF_B>(L.addr[EO + j]));   // 4 + (s_j // t_ji) * w_ji * p_ji
     const int img = (int)acc - 4 * EN;                                  // the image K_i (:66-68)
     tg[NI] = (u32)min(max(img, 0), 2);                                  // as far as the allowable states go (:70)
-    const bool told = tg[NI] != s[NI];
-    const bool eligible = told && cnt[NI] >= ((L.nb[NI] >> 4) & 3u);    // memory criterion (:79)
-    pr[NI] = eligible ? (L.nb[NI] & 15u) * (t - last[NI]) : 0u;         // speed x time steps since last updated (:82)
+    const bool eligible = tg[NI] != s[NI] && cnt[NI] >= L.m[NI];        // told to update, memory criterion met (:79, :82)
+    pr[NI] = eligible ? L.u[NI] * (t - last[NI]) : 0u;                  // speed x time steps since last updated (:82)
     top = max(top, pr[NI]);
-    Images<NI + 1>::run(L, rb, t, s, last, cnt, tg, pr, top);
+    Images<NI + 1, RB>::run(L, t, s, last, cnt, tg, pr, top);
   }
 };
-template <>
-struct Images<NS> {
-  static __device__ __forceinline__ void run(const Lane&, u32, u32, const u32 (&)[NS], const u32 (&)[NS], const u32 (&)[NS], u32 (&)[NS],
+template <int RB>
+struct Images<NS, RB> {
+  static __device__ __forceinline__ void run(const Lane&, u32, const u32 (&)[NS], const u32 (&)[NS], const u32 (&)[NS], u32 (&)[NS],
                                              u32 (&)[NS], u32&) {}
 };
+
+// the lane's cost tables of one time point: byte s+1 of word n = |s - r| * (|g| + 1) for its node slot n
+__device__ __forceinline__ void load_cost(const u32* row, u32 (&c)[NSP]) {
+  if constexpr (NSP == 1) { c[0] = __ldg(row); }
+  else if constexpr (NSP == 2) { const uint2 v = __ldg((const uint2*)row); c[0] = v.x; c[1] = v.y; }
+  else {
+#pragma unroll
+    for (int i = 0; i < NSP; i += 4) { const uint4 v = __ldg((const uint4*)(row + i)); c[i] = v.x; c[i + 1] = v.y; c[i + 2] = v.z; c[i + 3] = v.w; }
+  }
+}
+
+// One transition t-1 -> t reading state buffer RB and publishing into the other one,
+// and row t of the objective (:104-111).
+template <int RB, bool DUMP>
+__device__ __forceinline__ void transition(const Lane& L, u32 t, const u32* cost_row, u32 (&s)[NS], u32 (&last)[NS], u32 (&cnt)[NS],
+                                           u32& y, u8* dump_row) {
+  u32 cost[NSP];
+  load_cost(cost_row, cost);
+  u32 tg[NS], pr[NS];
+  u32 top = 0u;
+  Images<0, RB>::run(L, t, s, last, cnt, tg, pr, top);
+  top = group_max(top);
+#pragma unroll
+  for (int n = 0; n < NS; ++n) {
+    const int delta = (int)tg[n] - (int)s[n];
+    const bool mv = pr[n] == top && pr[n] != 0u;                      // the nodes sharing the highest priority (:82)
+    const int step = min(max(delta, -L.d[n]), L.d[n]);                // at most d_i levels toward K_i (:80)
+    s[n] = (u32)((int)s[n] + (mv ? step : 0));
+    last[n] = mv ? t : last[n];
+    cnt[n] = (delta != 0 && !mv) ? cnt[n] + 1u : 0u;                  // consecutive time steps told to update without moving
+    const u32 sel = kSel0 + s[n];
+    sts_u8<(1 - RB) * BUF_B>(L.self[n], sel);
+    y += prmt(cost[n], sel);                                          // |S - R| (.) (|G| + 1)  (:104-111)
+    if (DUMP && dump_row != nullptr && L.node[n] >= 0) dump_row[L.node[n]] = (u8)s[n];
+  }
+  __syncwarp();
+}
 
 // Simulate(x) (§2.1-2.3): the objective of the vector now in the lanes' registers.
 template <bool DUMP>
@@ -159,41 +218,29 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Lane& L, int lig,
   for (int k = 0; k < K; ++k) {
     u32 s[NS], last[NS], cnt[NS];
     const u32 iw = __ldg(p.init_lane + k * LPC + lig);
-    u32 rw = __ldg(p.ref_lane + (size_t)(k * (T + 1)) * LPC + lig);
-#pragma unroll
-    for (int n = 0; n < NS; ++n) {
-      s[n] = (iw >> (2 * n)) & 3u; last[n] = 0u; cnt[n] = 0u;
-      sts_u16(L.self[n], 0x4440u | s[n]);
-      const u32 r = (rw >> (4 * n)) & 3u, wgt = (rw >> (4 * n + 2)) & 3u;
-      y += (u32)abs((int)s[n] - (int)r) * wgt;                        // row t0 of S, R and G (:92-100)
-      if (DUMP && dump != nullptr && L.node[n] >= 0) dump[(size_t)(k * (T + 1)) * N + L.node[n]] = (u8)s[n];
-    }
-    __syncwarp();
-#pragma unroll 1
-    for (int t = 1; t <= T; ++t) {
-      const u32 rb = (u32)((t - 1) & 1) * BUF_B, wb = (u32)(t & 1) * BUF_B;
-      rw = __ldg(p.ref_lane + (size_t)(k * (T + 1) + t) * LPC + lig);
-      u32 tg[NS], pr[NS];
-      u32 top = 0u;
-      Images<0>::run(L, rb, (u32)t, s, last, cnt, tg, pr, top);
-      top = group_max(top);
+    const u32* cost_row = p.cost_lane + ((size_t)(k * (T + 1)) * LPC + lig) * NSP;
+    u8* dump_row = (DUMP && dump != nullptr) ? dump + (size_t)(k * (T + 1)) * N : nullptr;
+    {
+      u32 cost[NSP];
+      load_cost(cost_row, cost);
 #pragma unroll
       for (int n = 0; n < NS; ++n) {
-        const bool told = tg[n] != s[n];
-        const bool mv = pr[n] == top && pr[n] != 0u;                    // the nodes sharing the highest priority (:82)
-        const int dist = abs((int)tg[n] - (int)s[n]);
-        const int step = min(dist, (int)(L.nb[n] >> 6));                // at most d_i levels toward K_i (:80)
-        const u32 moved = tg[n] > s[n] ? s[n] + (u32)step : s[n] - (u32)step;
-        s[n] = mv ? moved : s[n];
-        last[n] = mv ? (u32)t : last[n];
-        cnt[n] = mv ? 0u : told ? cnt[n] + 1u : 0u;
-        sts_u16(L.self[n] + wb, 0x4440u | s[n]);
-        const u32 r = (rw >> (4 * n)) & 3u, wgt = (rw >> (4 * n + 2)) & 3u;
-        y += (u32)abs((int)s[n] - (int)r) * wgt;                      // |S - R| (.) (|G| + 1)  (:104-111)
-        if (DUMP && dump != nullptr && L.node[n] >= 0) dump[(size_t)(k * (T + 1) + t) * N + L.node[n]] = (u8)s[n];
+        s[n] = (iw >> (2 * n)) & 3u; last[n] = 0u; cnt[n] = 0u;
+        const u32 sel = kSel0 + s[n];
+        sts_u8<0>(L.self[n], sel);
+        y += prmt(cost[n], sel);                                      // row t0 of S, R and G (:92-100)
+        if (DUMP && dump_row != nullptr && L.node[n] >= 0) dump_row[L.node[n]] = (u8)s[n];
       }
-      __syncwarp();
     }
+    __syncwarp();
+    u32 t = 1u;
+#pragma unroll 1
+    for (; t + 1u <= (u32)T; t += 2u) {                               // two transitions per trip: the buffer roles are constants
+      transition<0, DUMP>(L, t, cost_row + (size_t)t * LPC * NSP, s, last, cnt, y, DUMP && dump_row ? dump_row + (size_t)t * N : nullptr);
+      transition<1, DUMP>(L, t + 1u, cost_row + (size_t)(t + 1u) * LPC * NSP, s, last, cnt, y,
+                          DUMP && dump_row ? dump_row + (size_t)(t + 1u) * N : nullptr);
+    }
+    if (T & 1) transition<0, DUMP>(L, (u32)T, cost_row + (size_t)T * LPC * NSP, s, last, cnt, y, DUMP && dump_row ? dump_row + (size_t)T * N : nullptr);
   }
   return group_sum(y);
 }
@@ -302,9 +349,9 @@ __device__ __forceinline__ void set_param(Lane& L, const ChainMem& m, const Prop
   } else {
     const int i = r.q - 3 * E - (r.cls - kU) * N;
     const int u = r.cls == kU ? v : m.canon[3 * E + i], mm = r.cls == kM ? v : m.canon[3 * E + N + i], d = r.cls == kD ? v : m.canon[3 * E + 2 * N + i];
-    const u32 nb = make_nb(u, mm, d);
 #pragma unroll
-    for (int n = 0; n < NS; ++n) if (mine && n == sel) L.nb[n] = nb;
+    for (int n = 0; n < NS; ++n)
+      if (mine && n == sel) { L.u[n] = (u32)u; L.m[n] = (u32)mm; L.d[n] = d; }
   }
 }
 

@@ -22,11 +22,11 @@ enum { kW = 0, kP = 1, kT = 2, kU = 3, kM = 4, kD = 5 };
 struct Params {
   // problem tables, identical for every chain
   const u32* ploc;        // [NP]
-  const u16* slot_src;    // [ES][LPC] byte offset, in a chain's state buffer, of the source node's selector
+  const u16* slot_src;    // [ES][LPC] byte offset (= position), in a chain's state buffer, of the source node's selector
   const int* slot_edge;   // [ES][LPC] caller edge id of the lane's edge slot, -1 = empty slot
   const int* pos_node;    // [NS][LPC] node id of the lane's node slot, -1 = padding
   const u32* init_lane;   // [K][LPC]  initial states of the lane's nodes, 2 bits per node slot
-  const u32* ref_lane;    // [K][T+1][LPC] per node slot 4 bits: reference value | (|g|+1) << 2, weight 0 = not measured
+  const u32* cost_lane;   // [K][T+1][LPC][NSP] per node slot (padded to 1, 2, 4 or 8): byte s+1 = |s - r| * (|g| + 1), 0 if not measured
   const u8* fast;         // [N] 1 = speed range {10,11,12}
   const int* in_ptr;      // [N+1] CSR by destination over caller edge ids (ascending)
   const int* in_edge;     // [E]

@@ -9,8 +9,8 @@
 
 namespace tsa {
 
-int build_paper_plan(const sap_network* net, const sap_observations* obs, bool need_ref, bool constrained, PaperPlan* out,
-                     std::string* err) {
+int build_paper_plan(const sap_network* net, const sap_observations* obs, bool need_ref, bool constrained, int64_t n_chains,
+                     int sm_count, PaperPlan* out, std::string* err) {
   auto fail = [&](const std::string& m) { *err = m; return SA_EINVAL; };
   if (!net || !obs) return fail("null argument");
   const int N = net->n_nodes, E = net->n_edges, K = obs->n_cond, T = obs->n_steps;
@@ -58,6 +58,8 @@ int build_paper_plan(const sap_network* net, const sap_observations* obs, bool n
 
   // lanes per chain, node slots; nodes sorted by in-degree so that a node slot holds nodes of similar degree
   pl.LPC = N <= 16 ? 8 : N <= 32 ? 16 : 32;
+  // measured on paper_mtb (63 nodes), R = 10 240: 32 lanes 407 M, 16 lanes 428 M, 8 lanes 290 M chain-steps/s
+  if (N > 32 && N <= 64 && n_chains / 2 >= 16LL * std::max(sm_count, 1)) pl.LPC = 16;
   if (const char* e = tsa::tune_env("TSA_PAPER_LPC")) {
     const int v = std::atoi(e);
     if ((v == 8 || v == 16 || v == 32) && 8 * v >= N) pl.LPC = v;
@@ -90,7 +92,7 @@ int build_paper_plan(const sap_network* net, const sap_observations* obs, bool n
     for (int x = pl.in_ptr[i]; x < pl.in_ptr[i + 1]; ++x) {
       const int e = pl.in_edge[x], k = eoff[n] + (x - pl.in_ptr[i]), s = pl.src[e];
       pl.slot_edge[(size_t)k * pl.LPC + l] = e;
-      pl.slot_src[(size_t)k * pl.LPC + l] = (uint16_t)(2 * (pl.node_slot[s] * pl.LPC + pl.node_lane[s]));
+      pl.slot_src[(size_t)k * pl.LPC + l] = (uint16_t)(pl.node_slot[s] * pl.LPC + pl.node_lane[s]);
       for (int cls = 0; cls < 3; ++cls)
         pl.ploc[(size_t)cls * E + e] = (uint32_t)cls | ((uint32_t)l << 3) | ((uint32_t)k << 8) | ((uint32_t)s << 16) | ((uint32_t)i << 24);
     }
@@ -102,7 +104,8 @@ int build_paper_plan(const sap_network* net, const sap_observations* obs, bool n
   for (int k = 0; k < K; ++k)
     for (int i = 0; i < N; ++i)
       pl.init_lane[(size_t)k * pl.LPC + pl.node_lane[i]] |= (uint32_t)obs->init_state[(size_t)k * N + i] << (2 * pl.node_slot[i]);
-  pl.ref_lane.assign((size_t)K * (T + 1) * pl.LPC, 0);
+  pl.NSP = pl.NS <= 1 ? 1 : pl.NS <= 2 ? 2 : pl.NS <= 4 ? 4 : 8;
+  pl.cost_lane.assign((size_t)K * (T + 1) * pl.LPC * pl.NSP, 0);
   if (obs->ref) {
     uint64_t scored = 0;
     for (int k = 0; k < K; ++k)
@@ -115,8 +118,9 @@ int build_paper_plan(const sap_network* net, const sap_observations* obs, bool n
             const uint8_t rp = obs->ref[((size_t)k * (T + 1) + t - 1) * N + i];
             if (rp != SA_UNOBSERVED) g = (int)r - (int)rp;
           }
-          const uint32_t field = (uint32_t)r | ((uint32_t)(std::abs(g) + 1) << 2);
-          pl.ref_lane[((size_t)k * (T + 1) + t) * pl.LPC + pl.node_lane[i]] |= field << (4 * pl.node_slot[i]);
+          uint32_t word = 0;                                 // byte s+1: |s - r| * (|g| + 1); byte 0 stays 0
+          for (int s = 0; s < 3; ++s) word |= (uint32_t)(std::abs(s - (int)r) * (std::abs(g) + 1)) << (8 * (s + 1));
+          pl.cost_lane[(((size_t)k * (T + 1) + t) * pl.LPC + pl.node_lane[i]) * pl.NSP + pl.node_slot[i]] = word;
           ++scored;
         }
     pl.max_objective = (uint32_t)std::min<uint64_t>(6 * scored, 0xFFFFFFFFull);

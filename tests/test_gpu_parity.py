@@ -123,44 +123,42 @@ def test_tiny_full_parity(B, problems_cache):
 
 
 def test_hpg_full_size_parity(B, problems_cache):
+    """HPG-shaped, ALL 1024 chains x 20 000 steps, full trace."""
     prob = problems_cache("hpg")
     sched = PB.default_schedule("hpg")                                # R = 1024, 20 000 steps
     orc = O.Oracle(prob)
-    chains = PB.spread_chains(1024, 48)
+    chains = list(range(1024))
     with Handle(B, prob, sched) as hd:
         B.sa_set_trace(hd.h, chains, 20000)
         B.sa_run(hd.h, 20000)
         check_chains(B, hd, orc, chains, 20000, B.sa_get_trace(hd.h, len(chains), 20000))
         check_all_fitness(B, hd, orc)
-    with Handle(B, prob, sched) as hd:                                # every chain, first 200 steps
-        B.sa_run(hd.h, 200)
-        check_chains(B, hd, orc, list(range(1024)), 200)
 
 
 def test_mtb_full_size_parity(B, problems_cache):
+    """Mtb-shaped, 32 chains (0-3 and 28 evenly spread) x 20 000 steps with trace; all
+    4096 chains x the first 20 steps."""
     prob = problems_cache("mtb")
     sched = PB.default_schedule("mtb")                                # R = 4096, 20 000 steps
     orc = O.Oracle(prob)
-    long_chains = [0, 4095]
-    short_chains = PB.spread_chains(4096, 14)
+    chains = sorted(set(PB.spread_chains(4096, 32) + [4095]))
+    assert len(chains) >= 32
     with Handle(B, prob, sched) as hd:
-        f0, _ = B.sa_get_fitness(hd.h, 4096)
-        B.sa_set_trace(hd.h, sorted(set(long_chains + short_chains)), 20000)
-        traced = sorted(set(long_chains + short_chains))
+        B.sa_set_trace(hd.h, chains, 20000)
         B.sa_run(hd.h, 20000)
-        trace = B.sa_get_trace(hd.h, len(traced), 20000)
-        check_chains(B, hd, orc, long_chains, 20000, trace[[traced.index(c) for c in long_chains]])
-        refs = oracle_chains(orc, sched, short_chains, 2500)          # trace prefix of more chains
-        for c, ref in zip(short_chains, refs):
-            assert np.array_equal(trace[traced.index(c)][:2500], ref["trace"]), f"chain {c}"
-            assert f0[c] == ref["init_fit"]
+        check_chains(B, hd, orc, chains, 20000, B.sa_get_trace(hd.h, len(chains), 20000))
         check_all_fitness(B, hd, orc)
     with Handle(B, prob, sched) as hd:                                # every chain, first 20 steps
+        f0, _ = B.sa_get_fitness(hd.h, 4096)
         B.sa_run(hd.h, 20)
+        refs = oracle_chains(orc, sched, list(range(4096)), 20)
+        assert f0.tolist() == [r["init_fit"] for r in refs]
         check_chains(B, hd, orc, list(range(4096)), 20)
 
 
 def test_scaling_chain_counts(B, problems_cache):
+    """per R 8 spread chains x 2000 steps, all chains x 2 steps, and chain c identical
+    across the three R (invariant vii)."""
     prob = problems_cache("mtb")
     orc = O.Oracle(prob)
     common = [0, 1, 500, 1023]
@@ -176,15 +174,15 @@ def test_scaling_chain_counts(B, problems_cache):
             traces[R] = {c: tr[chains.index(c)] for c in common}
             if R == 1024:
                 check_all_fitness(B, hd, orc)
+        with Handle(B, prob, sched) as hd:                            # all chains x 2 steps
+            B.sa_run(hd.h, 2)
+            check_chains(B, hd, orc, list(range(R)), 2)
     for c in common:                                                  # invariant (vii): independent of R
         assert np.array_equal(traces[1024][c], traces[8192][c]) and np.array_equal(traces[1024][c], traces[65536][c])
-    sched = PB.default_schedule("mtb", n_chains=65536, total_steps=PB.SCALING_STEPS)
-    with Handle(B, prob, sched) as hd:                                # all chains x 2 steps (sampled 1 in 16)
-        B.sa_run(hd.h, 2)
-        check_chains(B, hd, orc, list(range(0, 65536, 16)), 2)
 
 
 def test_large_parity(B, problems_cache):
+    """Large, 8 chains x 1000 steps with trace; all 2048 chains: initial fitness + 1 step."""
     prob = problems_cache("large")
     sched = PB.default_schedule("large")                              # R = 2048, 1000 steps
     orc = O.Oracle(prob)
@@ -199,7 +197,7 @@ def test_large_parity(B, problems_cache):
         check_chains(B, hd, orc, chains, 1000, B.sa_get_trace(hd.h, len(chains), 1000))
     with Handle(B, prob, sched) as hd:                                # all chains: one step
         B.sa_run(hd.h, 1)
-        check_chains(B, hd, orc, list(range(0, 2048, 4)), 1)
+        check_chains(B, hd, orc, list(range(2048)), 1)
 
 
 # --------------------------------------------------------------------------------- invariants
