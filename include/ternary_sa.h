@@ -61,7 +61,11 @@ typedef struct {
   const uint32_t *accept;                        /* [L][D]: floor(2^32 * exp(-d/T_l)), d = 1..D */
   uint32_t chain_id_base;                        /* global id of chain 0 (chain-range partition over
                                                     GPUs, reading 25); usually 0 */
+  uint32_t flags;                                /* SA_LEVEL_STATS or 0 (sa_create); sap_create takes its flags
+                                                    as an argument and ignores this field */
 } sa_schedule;
+
+#define SA_LEVEL_STATS 2u   /* count accepted / accepted-worse / new-best moves per temperature level */
 
 /* Parameter vector layout everywhere in this ABI: int8 params[E+N];
  *   params[e]     = weight of edge e (caller's edge order), in {-1,0,+1};
@@ -110,6 +114,12 @@ int sa_run_levels(sa_handle *h, int64_t n_levels, int32_t group_size);
 
 /* One chain's current and best vectors ([E+N] each) and fitnesses.  Any output may be NULL. */
 int sa_get_chain(sa_handle *h, int32_t chain, int8_t *cur, uint32_t *cur_fit, int8_t *best, uint32_t *best_fit);
+
+/* Acceptance statistics kept on the device by every kernel family (needs SA_LEVEL_STATS in sched->flags):
+ * stats [L][4] = per level of the schedule (the last one absorbing steps past it), summed over all chains
+ * since sa_create: steps, accepted moves, accepted moves with delta_cand > delta_cur ("worse solutions
+ * that are temporarily accepted"), new bests.  Synchronises the stream. */
+int sa_get_level_stats(sa_handle *h, uint64_t *stats);
 
 /* All chains' current / best fitness, [R] each.  Either may be NULL. */
 int sa_get_fitness(sa_handle *h, uint32_t *cur_fit, uint32_t *best_fit);

@@ -20,12 +20,13 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_imma_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info",
+           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info", "sa_get_level_stats",
            "sap_create", "sap_run", "sap_run_levels", "sap_best", "sap_destroy", "sap_eval", "sap_simulate",
            "sap_get_chain", "sap_get_fitness", "sap_set_trace", "sap_get_trace", "sap_get_level_stats", "sap_get_info",
            "sap_set_stream", "sap_jit_check")
 SAP_CONSTRAINED, SAP_LEVEL_STATS = 1, 2
 SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
+SA_LEVEL_STATS = 2
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2506_19866_b200.build` "
@@ -53,7 +54,7 @@ class _Observations(C.Structure):
 class _Schedule(C.Structure):
     _fields_ = [("n_chains", C.c_int32), ("seed", C.c_uint64), ("n_levels", C.c_int32),
                 ("steps_per_level", C.c_int32), ("dmax", C.c_int32), ("accept", C.c_void_p),
-                ("chain_id_base", C.c_uint32)]
+                ("chain_id_base", C.c_uint32), ("flags", C.c_uint32)]
 
 
 ALLOC_FN = C.CFUNCTYPE(C.c_void_p, C.c_size_t, C.c_void_p)
@@ -70,6 +71,7 @@ _lib.sa_eval.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
 _lib.sa_simulate.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.c_void_p, C.c_void_p]
 _lib.sa_get_chain.argtypes = [C.c_void_p, C.c_int32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.sa_get_fitness.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p]
+_lib.sa_get_level_stats.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_set_trace.argtypes = [C.c_void_p, C.c_void_p, C.c_int32, C.c_int64]
 _lib.sa_get_trace.argtypes = [C.c_void_p, C.c_void_p]
 _lib.sa_geometric_table.argtypes = [C.c_double, C.c_double, C.c_int32, C.c_int32, C.c_void_p]
@@ -178,12 +180,12 @@ def sa_geometric_table(t0: float, t_end: float, n_levels: int, dmax: int) -> np.
     return out
 
 
-def sa_create(prob, sched, stream: Optional[int] = None) -> int:
+def sa_create(prob, sched, stream: Optional[int] = None, flags: int = 0) -> int:
     """prob / sched: objects with the fields of problems.Problem / problems.Schedule.  Returns the handle."""
     net, obs, keep = _marshal_problem(prob)
     table = _arr(sched.accept, np.uint32)
     sc = _Schedule(sched.n_chains, sched.seed, sched.n_levels, sched.steps_per_level, sched.dmax,
-                   table.ctypes.data, getattr(sched, "chain_id_base", 0))
+                   table.ctypes.data, getattr(sched, "chain_id_base", 0), flags)
     h = C.c_void_p()
     _check(_lib.sa_create(C.byref(net), C.byref(obs), C.byref(sc), C.byref(h)), "sa_create")
     if stream is None and _hooks is not None:
@@ -246,6 +248,13 @@ def sa_get_fitness(h: int, n_chains: int):
     best = np.zeros(n_chains, dtype=np.uint32)
     _check(_lib.sa_get_fitness(h, cur.ctypes.data, best.ctypes.data), "sa_get_fitness")
     return cur, best
+
+
+def sa_get_level_stats(h: int, n_levels: int) -> dict:
+    out = np.zeros((n_levels, 4), dtype=np.uint64)
+    _check(_lib.sa_get_level_stats(h, out.ctypes.data), "sa_get_level_stats")
+    return {"steps": out[:, 0].astype(np.int64), "accepted": out[:, 1].astype(np.int64),
+            "accepted_worse": out[:, 2].astype(np.int64), "improved": out[:, 3].astype(np.int64)}
 
 
 def sa_set_trace(h: int, chains: Sequence[int], max_steps: int) -> None:
@@ -334,7 +343,7 @@ def sap_create(prob, sched, flags: int = 0, stream: Optional[int] = None) -> int
     net, obs, keep = _marshal_paper(prob)
     table = _arr(sched.accept, np.uint32)
     sc = _Schedule(sched.n_chains, sched.seed, sched.n_levels, sched.steps_per_level, sched.dmax,
-                   table.ctypes.data, getattr(sched, "chain_id_base", 0))
+                   table.ctypes.data, getattr(sched, "chain_id_base", 0), 0)
     h = C.c_void_p()
     _check(_lib.sap_create(C.byref(net), C.byref(obs), C.byref(sc), flags, C.byref(h)), "sap_create")
     if stream is None and _hooks is not None:

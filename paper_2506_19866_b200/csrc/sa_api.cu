@@ -186,6 +186,7 @@ tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
   q.key0 = h->S.key0; q.key1 = h->S.key1; q.chain_id_base = h->S.chain_id_base;
   q.n_levels = h->S.n_levels; q.dmax = h->S.dmax; q.steps_per_level = h->S.steps_per_level;
   q.accept = h->S.accept;
+  q.level_stats = h->S.level_stats;
   q.trace_row = h->Tr.row_of_chain; q.trace_rec = (tsa_dense::u64*)h->Tr.records;
   q.trace_max = h->Tr.max_steps; q.trace_g0 = h->Tr.g_start;
   q.g0 = h->g; q.steps = steps;
@@ -219,6 +220,7 @@ tsa_static::Params static_params(const sa_handle* h, int64_t steps) {
   q.key0 = h->S.key0; q.key1 = h->S.key1; q.chain_id_base = h->S.chain_id_base;
   q.n_levels = h->S.n_levels; q.dmax = h->S.dmax; q.steps_per_level = h->S.steps_per_level;
   q.accept = h->S.accept;
+  q.level_stats = h->S.level_stats;
   q.trace_row = h->Tr.row_of_chain; q.trace_rec = (tsa_static::u64*)h->Tr.records;
   q.trace_max = h->Tr.max_steps; q.trace_g0 = h->Tr.g_start;
   q.g0 = h->g; q.steps = steps;
@@ -321,6 +323,13 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
   {
     std::vector<uint32_t> tab(sched->accept, sched->accept + (size_t)sched->n_levels * sched->dmax);
     if ((rc = h->pool.upload(tab, &S.accept, st))) return rc;
+  }
+  S.level_stats = nullptr;
+  if (sched->flags & ~SA_LEVEL_STATS) return set_err(SA_EINVAL, "unknown schedule flag");
+  if (sched->flags & SA_LEVEL_STATS) {
+    S.level_stats = (unsigned long long*)h->pool.alloc((size_t)sched->n_levels * 4 * 8, st);
+    if (!S.level_stats) return set_err(SA_ENOMEM, "device allocation failed (level statistics)");
+    TSA_CUDA(cudaMemsetAsync(S.level_stats, 0, (size_t)sched->n_levels * 4 * 8, st));
   }
   std::memset(&h->Tr, 0, sizeof(h->Tr));
 
@@ -443,6 +452,14 @@ int sa_get_fitness(sa_handle* h, uint32_t* cur_fit, uint32_t* best_fit) {
   const size_t bytes = (size_t)h->C.R * 4;
   if (cur_fit) TSA_CUDA(cudaMemcpyAsync(cur_fit, h->C.fit_cur, bytes, cudaMemcpyDeviceToHost, h->stream));
   if (best_fit) TSA_CUDA(cudaMemcpyAsync(best_fit, h->C.fit_best, bytes, cudaMemcpyDeviceToHost, h->stream));
+  TSA_CUDA(cudaStreamSynchronize(h->stream));
+  return check_device_error(h);
+}
+
+int sa_get_level_stats(sa_handle* h, uint64_t* stats) {
+  if (!h || !stats) return set_err(SA_EINVAL, "null argument");
+  if (!h->S.level_stats) return set_err(SA_EINVAL, "the handle was created without SA_LEVEL_STATS");
+  TSA_CUDA(cudaMemcpyAsync(stats, h->S.level_stats, (size_t)h->S.n_levels * 4 * 8, cudaMemcpyDeviceToHost, h->stream));
   TSA_CUDA(cudaStreamSynchronize(h->stream));
   return check_device_error(h);
 }

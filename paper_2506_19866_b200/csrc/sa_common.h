@@ -69,6 +69,7 @@ struct DevSched {
   int n_levels, dmax;
   int64_t steps_per_level;
   const uint32_t* accept;        // device [L][D]
+  unsigned long long* level_stats;   // device [L][4] steps, accepted, accepted worse, new best; nullptr = off
 };
 
 struct DevTrace {

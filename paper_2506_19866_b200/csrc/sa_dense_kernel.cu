@@ -63,7 +63,7 @@ constexpr int kTUnroll = TSD_TUNROLL;           // unroll factor of the time loo
 constexpr bool SWZ = TSD_SWZ != 0;              // swizzled exchange buffer (KS = 4, one warp per chain): conflict-free stores AND loads
 constexpr int STATE_BYTES = SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
-constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 2) * 4 + 15) / 16 * 16;   // bytes per chain
+constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 8) * 4 + 15) / 16 * 16;   // bytes per chain
 constexpr u64 kObsLo = TSD_OBSMASK_LO, kObsHi = TSD_OBSMASK_HI;
 constexpr u32 kOnes = 0x01010101u, kTwos = 0x02020202u;
 constexpr bool kByteMism = NOBS * 2 * NW <= 255;   // mismatch counters stay in byte lanes
@@ -355,6 +355,15 @@ __device__ __forceinline__ void shift_threshold(const Params& p, Regs& r, u32 lo
 
 __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int ring_me, int ring_next);
 
+// add the piece's counts of level ctl[6] to the handle's table and clear them (one thread per chain)
+__device__ __noinline__ void flush_stats(const Params& p, volatile u32* ctl) {
+  if (ctl[2] != 0u) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) atomicAdd(p.level_stats + (size_t)ctl[6] * 4 + k, (u64)ctl[2 + k]);
+  }
+  ctl[2] = 0u; ctl[3] = 0u; ctl[4] = 0u; ctl[5] = 0u;
+}
+
 extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_dense(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) u32 smem_all[];
   const int tix = threadIdx.x % TEAM, wc = threadIdx.x / TEAM;       // thread within the chain's team, chain slot within the CTA
@@ -463,8 +472,9 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   // Chain control words live in shared memory and the proposal is derived a second time after the
   // simulation (from the step counter alone), so that nothing but the loop counter stays in
   // registers across the time loop: the register budget there decides warps per SM.
-  volatile u32* const ctl = red + 2 * TW;               // [0] d_cur, [1] d_best
-  if (tix == 0) { ctl[0] = __ldcg(p.fit_cur + chain); ctl[1] = __ldcg(p.fit_best + chain); }
+  volatile u32* const ctl = red + 2 * TW;               // [0] d_cur, [1] d_best, [2..5] steps / accepted / accepted worse / new best
+                                                        // of the level [6] this piece is running, thread 0 only
+  if (tix == 0) { ctl[0] = __ldcg(p.fit_cur + chain); ctl[1] = __ldcg(p.fit_best + chain); ctl[2] = 0u; ctl[6] = 0xFFFFFFFFu; }
   team_sync();
 
 #pragma unroll 1
@@ -487,6 +497,10 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     bool acc = d <= 0;
     if (!acc && d <= (i64)p.dmax) acc = q.x2 < __ldg(p.accept + level * (u64)p.dmax + (u64)(d - 1));
     const bool new_best = acc && fcand < fbest;
+    if (p.level_stats && tix == 0) {
+      if ((u32)level != ctl[6]) { flush_stats(p, ctl); ctl[6] = (u32)level; }
+      ctl[2] += 1u; ctl[3] += acc ? 1u : 0u; ctl[4] += (acc && d > 0) ? 1u : 0u; ctl[5] += new_best ? 1u : 0u;
+    }
     team_sync();                                         // everyone has read the control words
     // a6
     if (acc) {
@@ -521,7 +535,7 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   team_sync();
   for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)(p.cur_w + (size_t)chain * TSD_EPADA))[i] = ((const u32*)cw)[i];
   for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)(p.cur_th + (size_t)chain * TSD_NPADA))[i] = ((const u32*)cth)[i];
-  if (tix == 0) { p.fit_cur[chain] = ctl[0]; p.fit_best[chain] = ctl[1]; }
+  if (tix == 0) { p.fit_cur[chain] = ctl[0]; p.fit_best[chain] = ctl[1]; if (p.level_stats) flush_stats(p, ctl); }
   if (s1 < p.steps) {                        // hand the chain over
     __threadfence();
     team_sync();

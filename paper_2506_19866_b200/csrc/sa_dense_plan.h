@@ -31,7 +31,7 @@ struct DensePlan {
   std::vector<uint32_t> wloc;        // [E]
   std::vector<uint32_t> thloc;       // [N]
   size_t smem_bytes(const Plan& pl) const {   // per chain, as CHAIN_SMEM in the kernel
-    return ((size_t)(W > 1 ? 2 : 1) * (swizzle ? 1024 : 8 * CS) + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 2) * 4 + 15) / 16 * 16;
+    return ((size_t)(W > 1 ? 2 : 1) * (swizzle ? 1024 : 8 * CS) + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 8) * 4 + 15) / 16 * 16;
   }
 };
 

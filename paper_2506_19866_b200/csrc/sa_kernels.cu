@@ -371,6 +371,21 @@ __global__ void init_kernel(const DevProblem P, const DevChains C, const DevSche
 // SURVEY.md §8(c)-3).  Thread 0 of the team applies / reverts the one-byte mutation; every thread
 // computes the Philox block and the accept decision redundantly so no broadcast is needed.
 // ------------------------------------------------------------------------------------------
+// Acceptance statistics of one chain over the level it is running; added to the handle's [L][4] table
+// when the level ends and when the launch ends.
+struct LevelStats {
+  unsigned long long steps = 0, accepted = 0, worse = 0, best = 0;
+  __device__ __forceinline__ void count(bool acc, bool is_worse, bool new_best) {
+    steps += 1; accepted += acc; worse += acc && is_worse; best += new_best;
+  }
+  __device__ __forceinline__ void flush(unsigned long long* table, uint64_t lv) {
+    if (steps == 0) return;
+    atomicAdd(table + lv * 4 + 0, steps); atomicAdd(table + lv * 4 + 1, accepted);
+    atomicAdd(table + lv * 4 + 2, worse); atomicAdd(table + lv * 4 + 3, best);
+    steps = accepted = worse = best = 0;
+  }
+};
+
 template <int CG, typename Team, bool SMTAB>
 __device__ __forceinline__ void run_chain(const DevProblem& P, const Tables& tab, const Smem& sm, const DevChains& C,
                                           const DevSched& S, const DevTrace& Tr, const size_t chain,
@@ -386,6 +401,7 @@ __device__ __forceinline__ void run_chain(const DevProblem& P, const Tables& tab
 
   uint64_t level = g0 / (uint64_t)S.steps_per_level;
   int64_t left_in_level = S.steps_per_level - (int64_t)(g0 % (uint64_t)S.steps_per_level);
+  LevelStats stats;                 // acceptance statistics of the level being run, kept by the leader
   Team::sync();
 
   for (int64_t it = 0; it < steps; ++it) {
@@ -441,8 +457,13 @@ __device__ __forceinline__ void run_chain(const DevProblem& P, const Tables& tab
             ((uint64_t)(new_best ? 1 : 0) << 61);
       }
     }
-    if (--left_in_level == 0) { ++level; left_in_level = S.steps_per_level; }
+    if (S.level_stats && leader) stats.count(acc, d > 0, new_best);
+    if (--left_in_level == 0) {
+      if (S.level_stats && leader && level < (uint64_t)(S.n_levels - 1)) stats.flush(S.level_stats, lv);   // the last row absorbs the rest
+      ++level; left_in_level = S.steps_per_level;
+    }
   }
+  if (S.level_stats && leader) stats.flush(S.level_stats, level < (uint64_t)(S.n_levels - 1) ? level : (uint64_t)(S.n_levels - 1));
   Team::sync();
   // a7
   copy16<Team>(C.cur_w + chain * P.EpadA, sm.w, P.EpadA / 16);

@@ -332,6 +332,7 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
   const int trow = p.trace_row ? p.trace_row[chain] : -1;
   u64 level = p.g0 / (u64)p.steps_per_level;
   i64 left_in_level = p.steps_per_level - (i64)(p.g0 % (u64)p.steps_per_level);
+  u64 st_steps = 0, st_acc = 0, st_worse = 0, st_best = 0;    // acceptance statistics of the level being run
   team_sync();
 
 #pragma unroll 1
@@ -393,7 +394,22 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
         p.trace_rec[(size_t)trow * (size_t)p.trace_max + idx] =
             (u64)fcand | ((u64)pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61);
     }
-    if (--left_in_level == 0) { ++level; left_in_level = p.steps_per_level; }
+    if (p.level_stats) { st_steps += 1; st_acc += acc; st_worse += acc && d > 0; st_best += new_best; }
+    if (--left_in_level == 0) {
+      if (p.level_stats && level < (u64)(p.n_levels - 1)) {            // the last row absorbs the steps past the schedule
+        if (threadIdx.x == 0) {
+          atomicAdd(p.level_stats + lv * 4 + 0, st_steps); atomicAdd(p.level_stats + lv * 4 + 1, st_acc);
+          atomicAdd(p.level_stats + lv * 4 + 2, st_worse); atomicAdd(p.level_stats + lv * 4 + 3, st_best);
+        }
+        st_steps = st_acc = st_worse = st_best = 0;
+      }
+      ++level; left_in_level = p.steps_per_level;
+    }
+  }
+  if (p.level_stats && threadIdx.x == 0 && st_steps) {
+    const u64 lv = level < (u64)(p.n_levels - 1) ? level : (u64)(p.n_levels - 1);
+    atomicAdd(p.level_stats + lv * 4 + 0, st_steps); atomicAdd(p.level_stats + lv * 4 + 1, st_acc);
+    atomicAdd(p.level_stats + lv * 4 + 2, st_worse); atomicAdd(p.level_stats + lv * 4 + 3, st_best);
   }
   // a7
   RowIO<0>::store(r, cur_w, cur_th, warp, lane);

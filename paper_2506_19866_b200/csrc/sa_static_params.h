@@ -49,6 +49,8 @@ struct Params {
   u64* trace_rec;         // [n][trace_max]
   i64 trace_max;
   u64 trace_g0;
+  // acceptance statistics per temperature level (nullptr: off): [L][4] = steps, accepted, accepted worse, new best
+  u64* level_stats;
   // this launch
   u64 g0;
   i64 steps;
