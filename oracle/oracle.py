@@ -15,7 +15,10 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "sa_oracle.cpp")
-_LIB = os.path.join(_HERE, "libsa_oracle.so")
+# ORACLE_CXXFLAGS="-fsanitize=address,undefined -g": an instrumented copy of the oracle for the pin tests
+# (run them with LD_PRELOAD=$(g++ -print-file-name=libasan.so)); it is built beside the plain one
+_EXTRA = os.environ.get("ORACLE_CXXFLAGS", "").split()
+_LIB = os.path.join(_HERE, "libsa_oracle_san.so" if _EXTRA else "libsa_oracle.so")
 _lib = None
 
 
@@ -24,7 +27,7 @@ def build(force: bool = False) -> str:
     stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
     if force or stale:
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", tmp, _SRC])
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC"] + _EXTRA + ["-o", tmp, _SRC])
         os.replace(tmp, _LIB)
     return _LIB
 

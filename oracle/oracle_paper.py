@@ -15,7 +15,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRCS = [os.path.join(_HERE, "sa_oracle_paper.cpp"), os.path.join(_HERE, "sa_oracle.cpp")]
-_LIB = os.path.join(_HERE, "libsa_oracle_paper.so")
+_EXTRA = os.environ.get("ORACLE_CXXFLAGS", "").split()        # see oracle.py
+_LIB = os.path.join(_HERE, "libsa_oracle_paper_san.so" if _EXTRA else "libsa_oracle_paper.so")
 _lib = None
 
 
@@ -24,7 +25,7 @@ def build(force: bool = False) -> str:
     stale = (not os.path.exists(_LIB)) or any(os.path.getmtime(_LIB) < os.path.getmtime(s) for s in _SRCS)
     if force or stale:
         tmp = _LIB + ".tmp.%d" % os.getpid()
-        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC", "-o", tmp] + _SRCS)
+        subprocess.check_call(["g++", "-O2", "-std=c++17", "-shared", "-fPIC"] + _EXTRA + ["-o", tmp] + _SRCS)
         os.replace(tmp, _LIB)
     return _LIB
 
