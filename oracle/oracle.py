@@ -62,6 +62,12 @@ def lib():
                                     C.c_int64, C.c_int, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                     C.c_void_p, C.c_void_p]
         L.orc_geometric_table.argtypes = [C.c_double, C.c_double, C.c_int, C.c_int, C.c_void_p]
+        L.orc_valid.restype = C.c_int
+        L.orc_valid.argtypes = [C.c_void_p, C.c_void_p]
+        L.orc_init_chain_c.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_void_p]
+        L.orc_propose_c.restype = C.c_int
+        L.orc_propose_c.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.orc_run_chain_c.argtypes = L.orc_run_chain.argtypes
         _lib = L
     return _lib
 
@@ -105,6 +111,7 @@ def unpack_trace(rec: np.ndarray):
         "code": ((rec >> np.uint64(56)) & np.uint64(0xF)).astype(np.int64),
         "accepted": ((rec >> np.uint64(60)) & np.uint64(1)).astype(bool),
         "new_best": ((rec >> np.uint64(61)) & np.uint64(1)).astype(bool),
+        "null_move": ((rec >> np.uint64(62)) & np.uint64(1)).astype(bool),
     }
 
 
@@ -175,19 +182,38 @@ class Oracle:
             list(ex.map(work, range(threads)))
         return out
 
-    def init_chain(self, seed: int, chain: int):
+    def init_chain(self, seed: int, chain: int, constrained: bool = False):
         x = np.zeros(self.P, dtype=np.int8)
-        lib().orc_init_chain(self.h, seed, chain, x.ctypes.data)
+        if constrained:
+            indeg = np.bincount(self._keep[1], minlength=self.N)
+            outdeg = np.bincount(self._keep[0], minlength=self.N)
+            if (indeg == 0).any() or (outdeg == 0).any():       # no valid vector exists
+                raise ValueError("constraints need an in-edge and an out-edge at every node")
+            lib().orc_init_chain_c(self.h, seed, chain, x.ctypes.data)
+        else:
+            lib().orc_init_chain(self.h, seed, chain, x.ctypes.data)
         return x, self.fitness(x)
 
-    def run_chain(self, sched, chain: int, n_steps: int, g0: int = 0, state=None, trace: bool = True):
+    def valid(self, params) -> bool:
+        """Structural constraints (a) and (b) of PAPER.md:186-199 in this model (reading C1)."""
+        return bool(lib().orc_valid(self.h, self._params(params).ctypes.data))
+
+    def propose_c(self, x0: int, x1: int, cur):
+        """Constrained GetCandidate -> (parameter index, new value, moved)."""
+        cur = self._params(cur)
+        p, nv = C.c_int32(), C.c_int32()
+        moved = lib().orc_propose_c(self.h, x0, x1, cur.ctypes.data, C.byref(p), C.byref(nv))
+        return p.value, nv.value, bool(moved)
+
+    def run_chain(self, sched, chain: int, n_steps: int, g0: int = 0, state=None, trace: bool = True,
+                  constrained: bool = False):
         """Advance global chain id ``chain`` by n_steps from step g0.
 
         state = (cur, best, fit_cur, fit_best) or None (= fresh chain).
         Returns dict(cur, best, fit_cur, fit_best, trace, init_fit).
         """
         if state is None:
-            cur, f0 = self.init_chain(sched.seed, chain)
+            cur, f0 = self.init_chain(sched.seed, chain, constrained)
             best, fc, fb = cur.copy(), f0, f0
         else:
             cur, best, fc, fb = state
@@ -197,23 +223,25 @@ class Oracle:
         fcur, fbest = C.c_uint32(fc), C.c_uint32(fb)
         tr = np.zeros(n_steps if trace else 0, dtype=np.uint64)
         table = np.ascontiguousarray(sched.accept, dtype=np.uint32)
-        lib().orc_run_chain(self.h, sched.seed, chain, g0, n_steps, sched.n_levels, sched.steps_per_level,
-                            sched.dmax, table.ctypes.data, cur.ctypes.data, best.ctypes.data,
-                            C.byref(fcur), C.byref(fbest), tr.ctypes.data if trace else None)
+        run = lib().orc_run_chain_c if constrained else lib().orc_run_chain
+        run(self.h, sched.seed, chain, g0, n_steps, sched.n_levels, sched.steps_per_level,
+            sched.dmax, table.ctypes.data, cur.ctypes.data, best.ctypes.data,
+            C.byref(fcur), C.byref(fbest), tr.ctypes.data if trace else None)
         return {"cur": cur, "best": best, "fit_cur": fcur.value, "fit_best": fbest.value,
                 "trace": tr, "init_fit": f0}
 
-    def run_chains(self, sched, chains: Iterable[int], n_steps: int, threads: int = 1, trace: bool = True):
+    def run_chains(self, sched, chains: Iterable[int], n_steps: int, threads: int = 1, trace: bool = True,
+                   constrained: bool = False):
         """Independent chains, optionally replicated over host threads (ctypes drops the GIL)."""
         chains = list(chains)
         if threads <= 1:
-            return [self.run_chain(sched, c, n_steps, trace=trace) for c in chains]
+            return [self.run_chain(sched, c, n_steps, trace=trace, constrained=constrained) for c in chains]
         with ThreadPoolExecutor(threads) as ex:
-            return list(ex.map(lambda c: self.run_chain(sched, c, n_steps, trace=trace), chains))
+            return list(ex.map(lambda c: self.run_chain(sched, c, n_steps, trace=trace, constrained=constrained), chains))
 
 
 def run_levels(orc: "Oracle", sched, n_chains: int, n_levels: int, group_size: int = 0, g0: int = 0,
-               states=None, threads: int = 1):
+               states=None, threads: int = 1, constrained: bool = False):
     """PAPER.md Table 1 (:125-155), the level structure around the chain step, statement by statement:
 
         while T > T_min:                                   # here: n_levels levels from step g0
@@ -233,13 +261,14 @@ def run_levels(orc: "Oracle", sched, n_chains: int, n_levels: int, group_size: i
     if states is None:
         states = []
         for c in range(R):
-            x, f = orc.init_chain(sched.seed, base + c)
+            x, f = orc.init_chain(sched.seed, base + c, constrained)
             states.append((x, x.copy(), f, f))
     g = g0
     assert g % sched.steps_per_level == 0, "levels start at level boundaries"
     for _ in range(n_levels):
         def advance(c):
-            out = orc.run_chain(sched, base + c, sched.steps_per_level, g0=g, state=states[c], trace=False)
+            out = orc.run_chain(sched, base + c, sched.steps_per_level, g0=g, state=states[c], trace=False,
+                                constrained=constrained)
             return (out["cur"], out["best"], out["fit_cur"], out["fit_best"])
         if threads > 1:
             with ThreadPoolExecutor(threads) as ex:

@@ -15,6 +15,10 @@
 // proposal/accept mapping arithmetic, the acceptance-table closed form, the all-zero-weights
 // closed form, invariants (i)-(viii), brute force over a 4-node / 6-edge network, and Philox
 // against ATen's independent implementation.  Nothing on the hot path is "parity unpinned".
+//
+// Round 2 adds, without touching any of the above, the structural constraints of PAPER.md §2.5.3 for this
+// model (orc_valid, orc_init_chain_c, orc_propose_c, orc_run_chain_c at the end of the file; DESIGN.md
+// readings C1-C3), pinned by tests/test_oracle_constraints.py.
 
 #include <cmath>
 #include <cstdint>
@@ -244,4 +248,122 @@ void orc_geometric_table(double t0, double t_end, int L, int D, uint32_t* out) {
   }
 }
 
+
+// ---------------------------------------------------------------------------------------------------
+// Structural constraints in the config model, where one signed weight stands for the
+// paper's weight and polarity (w = +1 is an active activator, w = -1 an active inhibitor, 0 no edge):
+//   (a) every node has an in-edge and an out-edge of non-zero weight  (:187-191),
+//   (b) every node has an in-edge with w = +1                         (:193-199).
+// Checked by scanning the whole vector (reading C1).  Threshold parameters are unconstrained.
+int orc_valid(const void* h, const int8_t* x) {
+  const Problem& P = *(const Problem*)h;
+  std::vector<int> in_nz(P.N, 0), out_nz(P.N, 0), act(P.N, 0);
+  for (int e = 0; e < P.E; ++e) {
+    if (x[e] != 0) { in_nz[P.dst[e]] += 1; out_nz[P.src[e]] += 1; }
+    if (x[e] == 1) act[P.dst[e]] += 1;
+  }
+  for (int i = 0; i < P.N; ++i)
+    if (in_nz[i] == 0 || out_nz[i] == 0 || act[i] == 0) return 0;
+  return 1;
+}
+
+// Initial vector under constraints (:201 "each thread is given a valid solution vector"; reading C3): the
+// unconstrained vector of init_chain, then a repair pass "by conditionals" with Philox(ctr = (i, 0, chain, 2))
+// = (y0..y3) for node i: first, for i = 0..N-1, a node without a +1 in-edge gets w = +1 on its
+// mulhi(y0, indeg)-th in-edge (caller's edge order); then, for i = 0..N-1, a node without a non-zero
+// out-edge gets w = 2 * mulhi(y3, 2) - 1 on its mulhi(y2, outdeg)-th out-edge.
+void orc_init_chain_c(const void* h, uint64_t seed, uint32_t chain, int8_t* x) {
+  const Problem& P = *(const Problem*)h;
+  init_chain(P, seed, chain, x);
+  uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  std::vector<std::vector<int>> out_edges(P.N);
+  for (int e = 0; e < P.E; ++e) out_edges[P.src[e]].push_back(e);
+  for (int i = 0; i < P.N; ++i) {
+    bool act = false;
+    for (int e : P.in_edges[i]) act = act || x[e] == 1;
+    if (act) continue;
+    uint32_t ctr[4] = {(uint32_t)i, 0u, chain, 2u}, y[4];
+    philox4x32_10(ctr, key, y);
+    x[P.in_edges[i][mulhi(y[0], (uint32_t)P.in_edges[i].size())]] = 1;
+  }
+  for (int i = 0; i < P.N; ++i) {
+    bool nz = false;
+    for (int e : out_edges[i]) nz = nz || x[e] != 0;
+    if (nz) continue;
+    uint32_t ctr[4] = {(uint32_t)i, 0u, chain, 2u}, y[4];
+    philox4x32_10(ctr, key, y);
+    x[out_edges[i][mulhi(y[2], (uint32_t)out_edges[i].size())]] = (int8_t)(2 * (int)mulhi(y[3], 2u) - 1);
+  }
+}
+
+// GetCandidate under constraints (:201 "by using conditionals when perturbing the weight or polarity
+// components"; reading C2): index as in propose(); for a weight the two other values are listed
+// cyclically after the old one (code+1, code+2 mod 3), those whose vector would break (a) or (b) are
+// struck, the new value is entry mulhi(x1, length) of the list; an empty list gives a null move
+// (*new_out = old value, returns 0).  With both values allowed this is propose().  Thresholds as in propose().
+int orc_propose_c(const void* h, uint32_t x0, uint32_t x1, const int8_t* cur, int32_t* p_out, int32_t* new_out) {
+  const Problem& P = *(const Problem*)h;
+  const int NP = P.E + P.N;
+  const int p = (int)mulhi(x0, (uint32_t)NP);
+  *p_out = p;
+  if (p >= P.E) {
+    int q, nv;
+    propose(x0, x1, NP, P.E, P.n_pairs, cur, &q, &nv);
+    *new_out = nv;
+    return 1;
+  }
+  const int code = cur[p] + 1;
+  std::vector<int8_t> cand(cur, cur + NP);
+  int list[2], len = 0;
+  for (int k = 1; k <= 2; ++k) {
+    const int v = (code + k) % 3 - 1;
+    cand[p] = (int8_t)v;
+    if (orc_valid(h, cand.data())) list[len++] = v;
+  }
+  if (len == 0) { *new_out = cur[p]; return 0; }
+  *new_out = list[mulhi(x1, (uint32_t)len)];
+  return 1;
+}
+
+// orc_run_chain with the constrained GetCandidate; trace bit 62 = null move.  Everything else (Philox
+// counter layout, roles of x0 / x1 / x2, level rule, accept test, strict-improvement best) as above.
+void orc_run_chain_c(const void* h, uint64_t seed, uint32_t chain, uint64_t g0, int64_t n_steps,
+                     int n_levels, int64_t steps_per_level, int D, const uint32_t* table,
+                     int8_t* cur, int8_t* best, uint32_t* fit_cur, uint32_t* fit_best, uint64_t* trace) {
+  const Problem& P = *(const Problem*)h;
+  const int NP = P.E + P.N;
+  uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  std::vector<int8_t> cand(NP);
+  for (int64_t it = 0; it < n_steps; ++it) {
+    uint64_t g = g0 + (uint64_t)it;
+    uint32_t ctr[4] = {(uint32_t)g, (uint32_t)(g >> 32), chain, 0u}, x[4];
+    philox4x32_10(ctr, key, x);
+    int32_t p, nv;
+    const int moved = orc_propose_c(h, x[0], x[1], cur, &p, &nv);
+    std::memcpy(cand.data(), cur, NP);
+    cand[p] = (int8_t)nv;
+    uint32_t f_cand = fitness(P, cand.data(), nullptr);
+    int64_t d = (int64_t)f_cand - (int64_t)*fit_cur;
+    uint64_t level = g / (uint64_t)steps_per_level;
+    if (level > (uint64_t)(n_levels - 1)) level = (uint64_t)(n_levels - 1);
+    bool acc = accept_move(d, x[2], table + level * (uint64_t)D, D);
+    bool new_best = false;
+    if (acc) {
+      std::memcpy(cur, cand.data(), NP);
+      *fit_cur = f_cand;
+      if (f_cand < *fit_best) {
+        std::memcpy(best, cand.data(), NP);
+        *fit_best = f_cand;
+        new_best = true;
+      }
+    }
+    if (trace) {
+      uint64_t code = (p < P.E) ? (uint64_t)(nv + 1) : (uint64_t)nv;
+      trace[it] = (uint64_t)f_cand | ((uint64_t)p << 32) | (code << 56) | ((uint64_t)(acc ? 1 : 0) << 60) |
+                  ((uint64_t)(new_best ? 1 : 0) << 61) | ((uint64_t)(moved ? 0 : 1) << 62);
+    }
+  }
+}
+
 } // extern "C"
+
