@@ -61,10 +61,16 @@ typedef struct {
   const uint32_t *accept;                        /* [L][D]: floor(2^32 * exp(-d/T_l)), d = 1..D */
   uint32_t chain_id_base;                        /* global id of chain 0 (chain-range partition over
                                                     GPUs, reading 25); usually 0 */
-  uint32_t flags;                                /* SA_LEVEL_STATS or 0 (sa_create); sap_create takes its flags
+  uint32_t flags;                                /* SA_CONSTRAINED | SA_LEVEL_STATS or 0 (sa_create); sap_create takes its flags
                                                     as an argument and ignores this field */
 } sa_schedule;
 
+#define SA_CONSTRAINED  1u   /* structural constraints of PAPER.md:186-201 in GetCandidate and at initialisation, in this
+                                model's terms (readings C1-C3): every node keeps an in- and an out-edge of
+                                non-zero weight and an in-edge of weight +1; a weight proposal chooses among the values
+                                that keep them (a null move if none does, trace bit 62); every chain starts from a
+                                valid vector.  Needs an in- and an out-edge at every node (SA_EINVAL otherwise).
+                                Kernel families: dense and generic (AUTO never picks the static one then). */
 #define SA_LEVEL_STATS 2u   /* count accepted / accepted-worse / new-best moves per temperature level */
 
 /* Parameter vector layout everywhere in this ABI: int8 params[E+N];
@@ -127,7 +133,8 @@ int sa_get_fitness(sa_handle *h, uint32_t *cur_fit, uint32_t *best_fit);
 /* Trace the next sa_run calls for `n` chains (local indices): one u64 record per traced chain
  * per step, up to max_steps steps counted from the step counter at the time of this call.
  * Record: bits 0-31 delta_cand, 32-55 parameter index p, 56-59 new value code (weight+1 or pair
- * index), bit 60 accepted, bit 61 new best.  n = 0 switches tracing off. */
+ * index), bit 60 accepted, bit 61 new best, bit 62 null move (SA_CONSTRAINED: no value of the weight keeps the
+ * constraints; the candidate is the current vector).  n = 0 switches tracing off. */
 int sa_set_trace(sa_handle *h, const int32_t *chains, int32_t n, int64_t max_steps);
 
 /* records [n][max_steps] (row order = order given to sa_set_trace); steps not yet run are 0. */

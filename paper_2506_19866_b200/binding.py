@@ -26,7 +26,7 @@ EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simula
            "sap_set_stream", "sap_jit_check")
 SAP_CONSTRAINED, SAP_LEVEL_STATS = 1, 2
 SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
-SA_LEVEL_STATS = 2
+SA_CONSTRAINED, SA_LEVEL_STATS = 1, 2
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2506_19866_b200.build` "

@@ -167,6 +167,7 @@ bool use_dense(sa_handle* h) {
       const int per_sm = (int)((h->C.R + h->sm_count - 1) / std::max(h->sm_count, 1));
       tune.dense_blocks = std::max(1, std::min(h->dplan.sparse ? 16 : 12, per_sm));
     }
+    tune.constrained = h->S.constrained ? 1 : 0;
     h->dk = tsa::dense_kernel_get(h->plan, h->dplan, tune, &h->dense_why);
   }
   return h->dk != nullptr;
@@ -177,6 +178,8 @@ tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
   std::memset(&q, 0, sizeof(q));
   q.frag_slot = h->d_frag_slot; q.meta = h->d_meta; q.th_entry = h->d_th_entry; q.init_frag = h->d_init_frag;
   q.obs_word = h->d_obs_word; q.fix = h->d_fix; q.wloc = h->d_dwloc; q.thloc = h->d_dthloc;
+  q.con_in_ptr = h->P.con_in_ptr; q.con_in_slot = h->P.con_in_slot; q.con_out_ptr = h->P.con_out_ptr;
+  q.con_out_slot = h->P.con_out_slot; q.edge_nodes = h->P.edge_nodes;
   std::memcpy(q.tha, h->P.tha, 16);
   std::memcpy(q.thb, h->P.thb, 16);
   q.fit_const = h->dplan.fit_const;
@@ -198,6 +201,7 @@ tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
 bool use_static(sa_handle* h) {
   const int fam = env_family(h->family);
   if (fam == SA_KERNEL_GENERIC || fam == SA_KERNEL_DENSE) return false;
+  if (h->S.constrained) { h->static_why = "the static kernel does not implement SA_CONSTRAINED"; return false; }
   if (!h->sk_tried) {
     h->sk_tried = true;
     h->sk = tsa::static_kernel_get(h->plan, tsa::StaticTuning::from_env(), &h->static_why);
@@ -277,6 +281,14 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
   if (dev_err == cudaSuccess) dev_err = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
   int rc = tsa::build_plan(net, obs, true, plan_options(sched->n_chains, h->sm_count), &h->plan, &err);
   if (rc != SA_OK) return set_err(rc, err);
+  if (sched->flags & ~(SA_LEVEL_STATS | SA_CONSTRAINED)) return set_err(SA_EINVAL, "unknown schedule flag");
+  if (sched->flags & SA_CONSTRAINED) {
+    std::vector<char> has_in(net->n_nodes, 0), has_out(net->n_nodes, 0);
+    for (int e = 0; e < net->n_edges; ++e) { has_in[net->edge_dst[e]] = 1; has_out[net->edge_src[e]] = 1; }
+    for (int i = 0; i < net->n_nodes; ++i)
+      if (!has_in[i] || !has_out[i])
+        return set_err(SA_EINVAL, "with constraints on every node needs an in-edge and an out-edge (PAPER.md:187-191)");
+  }
   if (dev_err != cudaSuccess) return cuda_err(dev_err, "cudaGetDevice");
   cudaStream_t st = h->stream;
   if ((rc = upload_problem(h->plan, h->pool, &h->P, st))) return rc;
@@ -325,7 +337,27 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(tab, &S.accept, st))) return rc;
   }
   S.level_stats = nullptr;
-  if (sched->flags & ~SA_LEVEL_STATS) return set_err(SA_EINVAL, "unknown schedule flag");
+  S.constrained = (sched->flags & SA_CONSTRAINED) ? 1u : 0u;
+  if (S.constrained) {
+    // CSR over in- / out-edges in ascending caller edge order, as slots of the canonical weight row
+    const int N = net->n_nodes, E = net->n_edges;
+    std::vector<int32_t> in_ptr(N + 1, 0), out_ptr(N + 1, 0), in_slot(E), out_slot(E);
+    std::vector<uint32_t> nodes(E);
+    for (int e = 0; e < E; ++e) { ++in_ptr[net->edge_dst[e] + 1]; ++out_ptr[net->edge_src[e] + 1]; }
+    for (int i = 0; i < N; ++i) { in_ptr[i + 1] += in_ptr[i]; out_ptr[i + 1] += out_ptr[i]; }
+    std::vector<int32_t> a(in_ptr.begin(), in_ptr.end() - 1), b(out_ptr.begin(), out_ptr.end() - 1);
+    for (int e = 0; e < E; ++e) {
+      in_slot[a[net->edge_dst[e]]++] = h->plan.slot_of_param[e];
+      out_slot[b[net->edge_src[e]]++] = h->plan.slot_of_param[e];
+      nodes[e] = (uint32_t)net->edge_src[e] | ((uint32_t)net->edge_dst[e] << 16);
+    }
+    if ((rc = h->pool.upload(in_ptr, &h->P.con_in_ptr, st))) return rc;
+    if ((rc = h->pool.upload(in_slot, &h->P.con_in_slot, st))) return rc;
+    if ((rc = h->pool.upload(out_ptr, &h->P.con_out_ptr, st))) return rc;
+    if ((rc = h->pool.upload(out_slot, &h->P.con_out_slot, st))) return rc;
+    if ((rc = h->pool.upload(nodes, &h->P.edge_nodes, st))) return rc;
+    TSA_CUDA(cudaStreamSynchronize(st));                 // the host vectors die with this block
+  }
   if (sched->flags & SA_LEVEL_STATS) {
     S.level_stats = (unsigned long long*)h->pool.alloc((size_t)sched->n_levels * 4 * 8, st);
     if (!S.level_stats) return set_err(SA_ENOMEM, "device allocation failed (level statistics)");
@@ -405,7 +437,7 @@ int sa_run(sa_handle* h, int64_t steps) {
     return SA_OK;
   }
   if (env_family(h->family) == SA_KERNEL_STATIC)
-    return set_err(h->plan.team_warps > 0 ? SA_ECUDA : SA_EINVAL, "static kernel unavailable: " + h->static_why);
+    return set_err(h->plan.team_warps > 0 && !h->S.constrained ? SA_ECUDA : SA_EINVAL, "static kernel unavailable: " + h->static_why);
   if (h->warp_cpb > 0)
     TSA_CUDA(tsa::launch_run_warp(h->P, h->C, h->S, h->Tr, h->g, steps, h->warp_cpb, h->stream));
   else

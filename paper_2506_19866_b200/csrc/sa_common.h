@@ -52,6 +52,14 @@ struct DevProblem {
   const uint32_t* obsm;          // [n_chunks][n_obs][n_entries][CG] 0x01 in scored byte lanes
   const uint32_t* fix;           // entries: bits 0-15 byte offset in the state buffer, 16-23 value
   const int8_t*   obs_idx_of_t;  // [T+1] observation index of time t or -1
+  // structural constraints (only filled when the handle was created with SA_CONSTRAINED):
+  // CSR over the nodes' in- / out-edges in ascending caller edge order, holding each edge's SLOT in the
+  // canonical weight row, and the end points of every caller edge
+  const int32_t*  con_in_ptr;    // [N+1]
+  const int32_t*  con_in_slot;   // [E]
+  const int32_t*  con_out_ptr;   // [N+1]
+  const int32_t*  con_out_slot;  // [E]
+  const uint32_t* edge_nodes;    // [E] src | dst << 16
   int8_t tha[kMaxPairs];         // -t_lo      per pair
   int8_t thb[kMaxPairs];         // -t_hi - 1  per pair
 };
@@ -70,6 +78,7 @@ struct DevSched {
   int64_t steps_per_level;
   const uint32_t* accept;        // device [L][D]
   unsigned long long* level_stats;   // device [L][4] steps, accepted, accepted worse, new best; nullptr = off
+  uint32_t constrained;          // 1 = constrained GetCandidate / initialisation
 };
 
 struct DevTrace {

@@ -44,6 +44,9 @@
 #define TSD_EARLY_OBS 0
 #define TSD_TUNROLL 1
 #endif
+#ifndef TSD_CONSTRAINED
+#define TSD_CONSTRAINED 0
+#endif
 
 namespace tsa_dense {
 
@@ -313,8 +316,38 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
 struct Proposal {
   u32 x2, pidx, loc, slot, wx;
   int oldv, newv, wsel;
-  bool is_w, mine;
+  bool is_w, mine, moved;
 };
+
+// GetCandidate for a weight under the structural constraints (readings C1, C2), by
+// the lane that holds the weight: the two other values are listed cyclically after the old one; "to 0" is struck
+// if the edge is the target's only non-zero in-edge or the source's only non-zero out-edge, "away from +1" if it
+// is the target's only activator; the new value is entry mulhi(x1, length) of what is left; nothing left = null
+// move (the old value).  cw = the chain's canonical weight row.
+__device__ __noinline__ int constrained_weight(const Params& p, const i8* cw, u32 pidx, int oldv, u32 x1, bool* moved) {
+  bool bar_zero = false, bar_nonplus = false;
+  if (oldv != 0) {
+    const u32 en = __ldg(p.edge_nodes + pidx);
+    const int src = (int)(en & 0xFFFFu), dst = (int)(en >> 16);
+    int in_nz = 0, act = 0, out_nz = 0;
+    for (int x = __ldg(p.con_in_ptr + dst); x < __ldg(p.con_in_ptr + dst + 1); ++x) {
+      const int v = cw[__ldg(p.con_in_slot + x)];
+      in_nz += v != 0; act += v == 1;
+    }
+    for (int x = __ldg(p.con_out_ptr + src); x < __ldg(p.con_out_ptr + src + 1); ++x) out_nz += cw[__ldg(p.con_out_slot + x)] != 0;
+    bar_zero = in_nz == 1 || out_nz == 1;
+    bar_nonplus = oldv == 1 && act == 1;
+  }
+  int first = 2, second = 2;                             // 2 = struck
+#pragma unroll
+  for (int k = 1; k <= 2; ++k) {
+    const int v = (oldv + 1 + k) % 3 - 1;
+    if (!((v == 0 && bar_zero) || (v != 1 && bar_nonplus))) { if (first == 2) first = v; else second = v; }
+  }
+  *moved = first != 2;
+  if (first == 2) return oldv;
+  return (second != 2 && __umulhi(x1, 2u) != 0u) ? second : first;
+}
 
 __device__ __forceinline__ Proposal propose(const Params& p, u64 gs, u32 gchain, int lane, int ww, int g, const i8* cw, const i8* cth) {
   Proposal q;
@@ -325,12 +358,13 @@ __device__ __forceinline__ Proposal propose(const Params& p, u64 gs, u32 gchain,
   q.is_w = q.pidx < (u32)TSD_NE;
   q.loc = q.is_w ? __ldg(p.wloc + q.pidx) : __ldg(p.thloc + (q.pidx - (u32)TSD_NE));
   q.slot = q.loc >> 16;
-  q.oldv = 0; q.newv = 0; q.wsel = -1; q.wx = 0u;
+  q.oldv = 0; q.newv = 0; q.wsel = -1; q.wx = 0u; q.moved = true;
   if (q.is_w) {
     q.mine = ((q.loc >> 9) & 31u) == (u32)lane && ((q.loc >> 14) & 3u) == (u32)ww;
     if (q.mine) {
       q.oldv = cw[q.slot];
-      q.newv = (q.oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;      // (code + 1 + r) mod 3 - 1, code = old + 1
+      if (TSD_CONSTRAINED) q.newv = constrained_weight(p, cw, q.pidx, q.oldv, x[1], &q.moved);
+      else q.newv = (q.oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;      // (code + 1 + r) mod 3 - 1, code = old + 1
       q.wsel = (int)(q.loc & 0x7Fu);
       q.wx = ((u32)(q.oldv ^ q.newv) & 0xFFu) << (8 * ((q.loc >> 7) & 3u));
     }
@@ -528,7 +562,8 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
       const u32 code = q.is_w ? (u32)(q.newv + 1) : (u32)q.newv;
       if (gs >= p.trace_g0 && idx < (u64)p.trace_max)
         p.trace_rec[(size_t)trow * (size_t)p.trace_max + idx] =
-            (u64)fcand | ((u64)q.pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61);
+            (u64)fcand | ((u64)q.pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61) |
+            ((u64)(q.moved ? 0 : 1) << 62);
     }
   }
   // a7

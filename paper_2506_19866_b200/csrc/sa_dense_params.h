@@ -26,6 +26,13 @@ struct Params {
   const u32* fix;         // [NFIX_ROUNDS][32] clamp fix-ups: bits 0-15 byte offset in the state buffer, 16-17 value, bit 31 valid
   const u32* wloc;        // [E]
   const u32* thloc;       // [N]
+  // structural constraints (kernels built with TSD_CONSTRAINED=1): CSR over the nodes' in- / out-edges holding each
+  // edge's offset in the canonical weight row, and the end points of every caller edge (src | dst << 16)
+  const int* con_in_ptr;  // [N+1]
+  const int* con_in_slot; // [E]
+  const int* con_out_ptr; // [N+1]
+  const int* con_out_slot;// [E]
+  const u32* edge_nodes;  // [E]
   i8 tha[16];             // -t_lo     per threshold pair
   i8 thb[16];             // -t_hi - 1 per threshold pair
   int fit_const;          // mismatches of clamped observed entries minus the always-counted unscored entries

@@ -356,6 +356,28 @@ __global__ void init_kernel(const DevProblem P, const DevChains C, const DevSche
     }
   }
   __syncthreads();
+  if (S.constrained && threadIdx.x == 0) {
+    // repair pass (reading C3): every node gets an activating in-edge, then a non-zero out-edge
+    for (int i = 0; i < P.N; ++i) {
+      const int a = __ldg(P.con_in_ptr + i), b = __ldg(P.con_in_ptr + i + 1);
+      bool act = false;
+      for (int x = a; x < b; ++x) act = act || sm.w[__ldg(P.con_in_slot + x)] == 1;
+      if (act) continue;
+      uint32_t y[4];
+      philox4x32_10((uint32_t)i, 0u, gchain, 2u, S.key0, S.key1, y);
+      sm.w[__ldg(P.con_in_slot + a + (int)__umulhi(y[0], (uint32_t)(b - a)))] = 1;
+    }
+    for (int i = 0; i < P.N; ++i) {
+      const int a = __ldg(P.con_out_ptr + i), b = __ldg(P.con_out_ptr + i + 1);
+      bool nz = false;
+      for (int x = a; x < b; ++x) nz = nz || sm.w[__ldg(P.con_out_slot + x)] != 0;
+      if (nz) continue;
+      uint32_t y[4];
+      philox4x32_10((uint32_t)i, 0u, gchain, 2u, S.key0, S.key1, y);
+      sm.w[__ldg(P.con_out_slot + a + (int)__umulhi(y[2], (uint32_t)(b - a)))] = (int8_t)(2 * (int)__umulhi(y[3], 2u) - 1);
+    }
+  }
+  __syncthreads();
   build_ab<CtaTeam>(P, sm);
   __syncthreads();
   const uint32_t f = team_sum<CtaTeam>(simulate<CG, false, CtaTeam, false>(P, tab, sm, nullptr), sm.red) + P.fit_const;
@@ -371,6 +393,36 @@ __global__ void init_kernel(const DevProblem P, const DevChains C, const DevSche
 // SURVEY.md §8(c)-3).  Thread 0 of the team applies / reverts the one-byte mutation; every thread
 // computes the Philox block and the accept decision redundantly so no broadcast is needed.
 // ------------------------------------------------------------------------------------------
+// GetCandidate for a weight under the structural constraints (readings C1, C2): the
+// two other values are listed cyclically after the old one; "to 0" is struck if the edge is the target's
+// only non-zero in-edge or the source's only non-zero out-edge, "away from +1" if it is the target's only
+// activator; the new value is entry mulhi(x1, length) of what is left; nothing left = null move (old value).
+// w = the chain's canonical weight row (slot order).  Executed by one thread.
+__device__ __forceinline__ int constrained_weight(const DevProblem& P, const int8_t* w, int p, int oldv, uint32_t x1, bool* moved) {
+  bool bar_zero = false, bar_nonplus = false;
+  if (oldv != 0) {
+    const uint32_t en = __ldg(P.edge_nodes + p);
+    const int src = (int)(en & 0xFFFFu), dst = (int)(en >> 16);
+    int in_nz = 0, act = 0, out_nz = 0;
+    for (int x = __ldg(P.con_in_ptr + dst); x < __ldg(P.con_in_ptr + dst + 1); ++x) {
+      const int v = w[__ldg(P.con_in_slot + x)];
+      in_nz += v != 0; act += v == 1;
+    }
+    for (int x = __ldg(P.con_out_ptr + src); x < __ldg(P.con_out_ptr + src + 1); ++x) out_nz += w[__ldg(P.con_out_slot + x)] != 0;
+    bar_zero = in_nz == 1 || out_nz == 1;
+    bar_nonplus = oldv == 1 && act == 1;
+  }
+  int list[2], len = 0;
+#pragma unroll
+  for (int k = 1; k <= 2; ++k) {
+    const int v = (oldv + 1 + k) % 3 - 1;
+    if (!((v == 0 && bar_zero) || (v != 1 && bar_nonplus))) list[len++] = v;
+  }
+  *moved = len > 0;
+  if (len == 0) return oldv;
+  return list[len == 2 ? (int)__umulhi(x1, 2u) : 0];
+}
+
 // Acceptance statistics of one chain over the level it is running; added to the handle's [L][4] table
 // when the level ends and when the launch ends.
 struct LevelStats {
@@ -411,11 +463,13 @@ __device__ __forceinline__ void run_chain(const DevProblem& P, const Tables& tab
     const int p = (int)__umulhi(x[0], (uint32_t)P.P);
     // a1/a2: the leader proposes and applies; (loc, old) let it revert
     int loc = 0, oldv = 0, newv = 0;
+    bool moved = true;
     if (leader) {
       if (p < P.E) {
         loc = __ldg(P.slot_of_param + p);
         oldv = sm.w[loc];
-        newv = (oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;          // (code + 1 + r) mod 3 - 1, code = old + 1
+        if (S.constrained) newv = constrained_weight(P, sm.w, p, oldv, x[1], &moved);
+        else newv = (oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;     // (code + 1 + r) mod 3 - 1, code = old + 1
         sm.w[loc] = (int8_t)newv;
       } else {
         loc = __ldg(P.entry_of_node + (p - P.E));
@@ -454,7 +508,7 @@ __device__ __forceinline__ void run_chain(const DevProblem& P, const Tables& tab
         const uint64_t code = (p < P.E) ? (uint64_t)(newv + 1) : (uint64_t)newv;
         Tr.records[(size_t)trow * Tr.max_steps + idx] =
             (uint64_t)fcand | ((uint64_t)p << 32) | (code << 56) | ((uint64_t)(acc ? 1 : 0) << 60) |
-            ((uint64_t)(new_best ? 1 : 0) << 61);
+            ((uint64_t)(new_best ? 1 : 0) << 61) | ((uint64_t)(moved ? 0 : 1) << 62);
       }
     }
     if (S.level_stats && leader) stats.count(acc, d > 0, new_best);

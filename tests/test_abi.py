@@ -77,6 +77,11 @@ def test_sa_create_validation(B, problems_cache):
     _bad(B, p, sched, "obs_times")
     s = copy.copy(sched); s.n_chains = 0
     _bad(B, good, s, "schedule")
+    # constraints need a closed loop: tiny has nodes without in-edges; unknown flags are refused
+    for flags, match in ((B.SA_CONSTRAINED, "in-edge"), (64, "flag")):
+        with pytest.raises(B.SaError) as ei:
+            B.sa_create(good, sched, flags=flags)
+        assert ei.value.code == B.SA_EINVAL and match in str(ei.value), str(ei.value)
     # accumulator range: a node with in-degree 63 is refused (reading 24)
     N = 65
     star = copy.copy(good)
