@@ -70,7 +70,7 @@ typedef struct {
                                 non-zero weight and an in-edge of weight +1; a weight proposal chooses among the values
                                 that keep them (a null move if none does, trace bit 62); every chain starts from a
                                 valid vector.  Needs an in- and an out-edge at every node (SA_EINVAL otherwise).
-                                Kernel families: dense and generic (AUTO never picks the static one then). */
+                                Every kernel family implements it. */
 #define SA_LEVEL_STATS 2u   /* count accepted / accepted-worse / new-best moves per temperature level */
 
 /* Parameter vector layout everywhere in this ABI: int8 params[E+N];

@@ -201,10 +201,11 @@ tsa_dense::Params dense_params(const sa_handle* h, int64_t steps) {
 bool use_static(sa_handle* h) {
   const int fam = env_family(h->family);
   if (fam == SA_KERNEL_GENERIC || fam == SA_KERNEL_DENSE) return false;
-  if (h->S.constrained) { h->static_why = "the static kernel does not implement SA_CONSTRAINED"; return false; }
   if (!h->sk_tried) {
     h->sk_tried = true;
-    h->sk = tsa::static_kernel_get(h->plan, tsa::StaticTuning::from_env(), &h->static_why);
+    tsa::StaticTuning tune = tsa::StaticTuning::from_env();
+    tune.constrained = h->S.constrained ? 1 : 0;
+    h->sk = tsa::static_kernel_get(h->plan, tune, &h->static_why);
   }
   return h->sk != nullptr;
 }
@@ -215,6 +216,8 @@ tsa_static::Params static_params(const sa_handle* h, int64_t steps) {
   q.lane_off2 = h->d_lane_off2; q.lane_meta = h->d_lane_meta; q.lane_clamp = h->d_lane_clamp;
   q.initw = h->P.initw; q.obsw = h->P.obsw; q.obsm = h->P.obsm;
   q.wloc = h->d_wloc; q.thloc = h->d_thloc;
+  q.con_in_ptr = h->P.con_in_ptr; q.con_in_slot = h->P.con_in_slot; q.con_out_ptr = h->P.con_out_ptr;
+  q.con_out_slot = h->P.con_out_slot; q.edge_nodes = h->P.edge_nodes;
   std::memcpy(q.tha, h->P.tha, 16);
   std::memcpy(q.thb, h->P.thb, 16);
   q.fit_const = h->P.fit_const;
@@ -437,7 +440,7 @@ int sa_run(sa_handle* h, int64_t steps) {
     return SA_OK;
   }
   if (env_family(h->family) == SA_KERNEL_STATIC)
-    return set_err(h->plan.team_warps > 0 && !h->S.constrained ? SA_ECUDA : SA_EINVAL, "static kernel unavailable: " + h->static_why);
+    return set_err(h->plan.team_warps > 0 ? SA_ECUDA : SA_EINVAL, "static kernel unavailable: " + h->static_why);
   if (h->warp_cpb > 0)
     TSA_CUDA(tsa::launch_run_warp(h->P, h->C, h->S, h->Tr, h->g, steps, h->warp_cpb, h->stream));
   else

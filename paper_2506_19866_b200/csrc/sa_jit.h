@@ -27,7 +27,7 @@ struct StaticTuning {
   int dense_swizzle = 1;  // dense kernel: swizzled exchange buffer when it applies
   int dense_sparse = 1;   // dense kernel: use the 2:4-sparse A operand (mma.sp) when the network allows it
   int dense_warps = 1;    // dense kernel: warps per chain (1, 2 or 4); 1 measured fastest at every R
-  int constrained = 0;    // dense kernel: build the constrained GetCandidate in (handles created with SA_CONSTRAINED)
+  int constrained = 0;    // static / dense kernel: build the constrained GetCandidate in (handles created with SA_CONSTRAINED)
   static StaticTuning from_env();
 };
 

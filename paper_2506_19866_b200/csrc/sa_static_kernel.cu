@@ -35,6 +35,10 @@
 #define TSA_TUNROLL 1
 #define TSA_BATCH 8
 #endif
+#ifndef TSA_CONSTRAINED
+#define TSA_CONSTRAINED 0
+#define TSA_NN 100
+#endif
 
 namespace tsa_static {
 
@@ -327,6 +331,23 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
   }
   const u32 sbase = (u32)__cvta_generic_to_shared(smem);
   u32* const red = smem + 3 * STATE_WORDS;
+  // structural constraints (readings C1, C2): per node the number of non-zero in-edges,
+  // non-zero out-edges and +1 in-edges of the chain's current vector, kept in shared memory behind the reduction
+  // words; only the thread that holds the proposed weight reads or writes them, between two team barriers
+  unsigned char* const cin = (unsigned char*)(red + W);
+  unsigned char* const cout = cin + TSA_NN;
+  unsigned char* const cact = cout + TSA_NN;
+  if (TSA_CONSTRAINED) {
+    for (int i = threadIdx.x; i < TSA_NN; i += TEAM) {
+      int a = 0, b = 0, c = 0;
+      for (int x = __ldg(p.con_in_ptr + i); x < __ldg(p.con_in_ptr + i + 1); ++x) {
+        const int v = cur_w[__ldg(p.con_in_slot + x)];
+        a += v != 0; c += v == 1;
+      }
+      for (int x = __ldg(p.con_out_ptr + i); x < __ldg(p.con_out_ptr + i + 1); ++x) b += cur_w[__ldg(p.con_out_slot + x)] != 0;
+      cin[i] = (unsigned char)a; cout[i] = (unsigned char)b; cact[i] = (unsigned char)c;
+    }
+  }
 
   u32 fcur = p.fit_cur[chain], fbest = p.fit_best[chain];
   const int trow = p.trace_row ? p.trace_row[chain] : -1;
@@ -347,12 +368,32 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
     const bool mine = (loc >> 16) == threadIdx.x;
     const int sel = mine ? (int)(loc & 0xFFu) : -1;
     u32 saved = 0u, code = 0u;
+    bool moved = true;
+    int dnz = 0, dact = 0, csrc = 0, cdst = 0;                          // constraint-counter changes if the move is accepted
     if (is_w) {
       const int sh = (int)((loc >> 8) & 3u) * 8;
 #pragma unroll
       for (int i = 0; i < NWREG; ++i) if (i == sel) saved = r.w[i];
       const int oldv = (int)(saved << (24 - sh)) >> 24;
-      const int newv = (oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;   // (code + 1 + r) mod 3 - 1, code = old + 1
+      int newv = (oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;         // (code + 1 + r) mod 3 - 1, code = old + 1
+      if (TSA_CONSTRAINED && mine) {
+        // the two other values, listed cyclically after the old one; strike "to 0" if the edge is the target's only
+        // non-zero in-edge or the source's only non-zero out-edge, "away from +1" if it is the target's only
+        // activator; take entry mulhi(x1, length) of what is left; nothing left = null move
+        const u32 en = __ldg(p.edge_nodes + pidx);
+        csrc = (int)(en & 0xFFFFu); cdst = (int)(en >> 16);
+        const bool bar_zero = oldv != 0 && (cin[cdst] == 1 || cout[csrc] == 1);
+        const bool bar_nonplus = oldv == 1 && cact[cdst] == 1;
+        int first = 2, second = 2;
+#pragma unroll
+        for (int k = 1; k <= 2; ++k) {
+          const int v = (oldv + 1 + k) % 3 - 1;
+          if (!((v == 0 && bar_zero) || (v != 1 && bar_nonplus))) { if (first == 2) first = v; else second = v; }
+        }
+        moved = first != 2;
+        newv = !moved ? oldv : (second != 2 && __umulhi(x[1], 2u) != 0u) ? second : first;
+        dnz = (newv != 0) - (oldv != 0); dact = (newv == 1) - (oldv == 1);
+      }
       const u32 neww = (saved & ~(0xFFu << sh)) | (((u32)newv & 0xFFu) << sh);
 #pragma unroll
       for (int i = 0; i < NWREG; ++i) if (i == sel) r.w[i] = neww;
@@ -376,6 +417,10 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
     // a6
     if (acc) {
       fcur = fcand;
+      if (TSA_CONSTRAINED && mine && is_w) {
+        cin[cdst] = (unsigned char)(cin[cdst] + dnz); cout[csrc] = (unsigned char)(cout[csrc] + dnz);
+        cact[cdst] = (unsigned char)(cact[cdst] + dact);
+      }
       if (fcand < fbest) {
         fbest = fcand;
         new_best = true;
@@ -392,7 +437,8 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
       const u64 idx = g - p.trace_g0;
       if (g >= p.trace_g0 && idx < (u64)p.trace_max)
         p.trace_rec[(size_t)trow * (size_t)p.trace_max + idx] =
-            (u64)fcand | ((u64)pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61);
+            (u64)fcand | ((u64)pidx << 32) | ((u64)code << 56) | ((u64)(acc ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61) |
+            ((u64)(moved ? 0 : 1) << 62);
     }
     if (p.level_stats) { st_steps += 1; st_acc += acc; st_worse += acc && d > 0; st_best += new_best; }
     if (--left_in_level == 0) {

@@ -28,6 +28,13 @@ struct Params {
   const u32* obsm;        // [NOBS][STATE_WORDS] 0x01 in scored byte lanes
   const u32* wloc;        // [E]  weight register | byte << 8 | thread << 16 holding edge e
   const u32* thloc;       // [N]  tier | thread << 16 of the lane that finalises node i
+  // structural constraints (kernels built with TSA_CONSTRAINED=1): CSR over the nodes' in- / out-edges holding each
+  // edge's offset in the canonical weight row, and the end points of every caller edge (src | dst << 16)
+  const int* con_in_ptr;  // [N+1]
+  const int* con_in_slot; // [E]
+  const int* con_out_ptr; // [N+1]
+  const int* con_out_slot;// [E]
+  const u32* edge_nodes;  // [E]
   i8 tha[16];             // -t_lo     per threshold pair
   i8 thb[16];             // -t_hi - 1 per threshold pair
   u32 fit_const;          // mismatches of clamped observed entries
