@@ -76,7 +76,13 @@ static_assert(!SWZ || (KS == 4 && TSD_W == 1), "the swizzled exchange buffer is 
 static_assert(2 * KS >= MT && MT >= 1, "row <-> column numbering needs MT <= 2*KS");
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
 static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
-static_assert(CPB == 1 || (TW == 1 && CPB % 4 == 0 && CPB <= 12), "several chains per CTA: one-warp chains, whole rings, at most 15 named barriers");
+static_assert(CPB == 1 || (TW == 1 && CPB % 4 == 0 && CPB <= 16), "several chains per CTA: one-warp chains, whole rings, at most 15 named barriers");
+// CPB <= 12: one token per warp (a ring of CPB/4 warps per SM sub-partition, barrier 1 + warp).  CPB == 16: the four
+// warps of a sub-partition form two PAIRS that take turns on the tensor pipe (barriers 1 + 2q and 2 + 2q): while one
+// pair issues its 2 x 14 IMMAs the other pair does its integer work, which is what keeps both the pipe and the issue
+// port busy (free-running warps fall into lock step: all in the tensor phase, then all in the integer phase).
+constexpr bool kPairs = CPB == 16;
+constexpr int kRingThreads = kPairs ? 128 : 64;
 
 // Philox4x32-10 (Salmon et al., SC'11)
 __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1, u32 (&out)[4]) {
@@ -148,8 +154,8 @@ __device__ __forceinline__ void sts_u8(u32 a, u32 v) { smem_check(a, 1); asm vol
 // half the time); instead the warp holding the token issues its IMMAs, passes the token on, and does
 // its integer work while the next warp uses the pipe.  One named barrier per warp, 64 threads:
 // the waiting warp's bar.sync and its predecessor's bar.arrive.
-__device__ __forceinline__ void ring_wait(int id) { asm volatile("bar.sync %0, 64;" ::"r"(id) : "memory"); }
-__device__ __forceinline__ void ring_pass(int id) { asm volatile("bar.arrive %0, 64;" ::"r"(id) : "memory"); }
+__device__ __forceinline__ void ring_wait(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(kRingThreads) : "memory"); }
+__device__ __forceinline__ void ring_pass(int id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "n"(kRingThreads) : "memory"); }
 
 // a[sel] ^= x for a run-time sel (a jump table: registers cannot be indexed); sel outside [0, NA) does nothing
 #define TSD_C1(i) case (i): if ((i) < NA) a[(i) < NA ? (i) : 0] ^= x; break;
@@ -408,9 +414,16 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
   if (CPB > 1) {
     const int q = wc & 3, pos = wc >> 2, G = CPB >= 4 ? CPB / 4 : 1;
     if (blockIdx.x * CPB + (u32)(q + 4 * (G - 1)) < (u32)p.R) {
-      ring_me = 1 + wc;
-      ring_next = 1 + q + 4 * ((pos + 1) % G);
-      if (pos == G - 1) ring_pass(ring_next);                        // the token starts at the ring's first warp
+      if (kPairs) {
+        const int pair = pos >> 1;                                     // warps q, q+4 are pair 0; q+8, q+12 pair 1
+        ring_me = 1 + 2 * q + pair;
+        ring_next = 1 + 2 * q + (1 - pair);
+        if (pair == 1) ring_pass(ring_next);                           // pair 0 goes first
+      } else {
+        ring_me = 1 + wc;
+        ring_next = 1 + q + 4 * ((pos + 1) % G);
+        if (pos == G - 1) ring_pass(ring_next);                        // the token starts at the ring's first warp
+      }
     }
     if (chain >= (u32)p.R) return;
   }

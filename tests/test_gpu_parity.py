@@ -247,7 +247,7 @@ FAMILY_CASES = [
     ("mtb", "GENERIC", {}), ("mtb", "STATIC", {}), ("mtb", "DENSE", {}),
     ("mtb", "DENSE", {"TSA_DENSE_W": "2"}), ("mtb", "DENSE", {"TSA_DENSE_W": "4"}),
     ("mtb", "DENSE", {"TSA_DENSE_BLOCKS": "8"}), ("mtb", "DENSE", {"TSA_DENSE_PH": "2"}),
-    ("mtb", "DENSE", {"TSA_DENSE_CPB": "8"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "12"}),
+    ("mtb", "DENSE", {"TSA_DENSE_CPB": "8"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "12"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "16"}),
     ("hpg", "DENSE", {"TSA_DENSE_CPB": "4"}),
     ("mtb", "DENSE", {"TSA_DENSE_SP": "0"}), ("mtb", "DENSE", {"TSA_DENSE_SP": "0", "TSA_DENSE_W": "2"}),
     ("mtb", "DENSE", {"TSA_DENSE_SP": "0", "TSA_DENSE_CPB": "8"}),
