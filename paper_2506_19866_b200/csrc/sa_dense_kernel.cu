@@ -10,10 +10,15 @@
 // the entire sa_run, every warp the states of t-1 as KS B fragments, and the team issues MT*KS IMMAs
 // per time step (v5: the 2:4-sparse form, mma.sp m16n8k64 -- half the registers and half the IMMAs; the
 // host permutes the nodes so that every row has at most two candidate edges per four columns).
-// The sums come back as C fragments, are packed four to a word (byte lanes), thresholded with
-// the same biased-byte trick as the gather kernel, and go through a 1-2 KB shared-memory buffer laid
-// out so that every lane writes its result words with one vector store and reads its next B
-// fragments with two vector loads (row <-> column numbering chosen by the host, sa_dense_plan.cpp).
+// Two row tiles share one accumulator (v7): the states travel as the bytes 64*s (0x00 / 0x40 / 0x80, an
+// unsigned B operand); the even tile of a pair multiplies s = (64*s) >> 6 by weights +-1, the odd tile
+// multiplies 64*s by weights +-4, so its sums arrive 256-fold: one s32 holds two sums a byte apart,
+// a word of four is ONE multiply-add of two accumulators, and only 2*MT accumulator registers are live.
+// The words are thresholded with the same biased-byte trick as the gather kernel (bit 7 of word + A is
+// [sum >= t_lo], bit 7 of word + A + D is [sum > t_hi]; three logic operations turn the two bits into
+// the byte 64*s') and go through a 1-2 KB shared-memory buffer laid out so that every lane writes its
+// result words with one vector store and reads its next B fragments with two vector loads (row <->
+// column numbering chosen by the host, sa_dense_plan.cpp).
 // Compiled at run time by NVRTC (sa_jit.cpp) with the problem's shape as -D constants, and ahead of
 // time with the Mtb-shaped defaults below (build check, SASS inspection).  It includes nothing:
 // sa_dense_params.h is prepended by whoever compiles it.
@@ -44,6 +49,17 @@
 #define TSD_EARLY_OBS 0
 #define TSD_TUNROLL 1
 #endif
+#ifndef TSD_IMMA_ORDER
+#define TSD_IMMA_ORDER 0
+#endif
+#ifndef TSD_IMMA_VOLATILE
+#define TSD_IMMA_VOLATILE 1
+#endif
+#if TSD_IMMA_VOLATILE
+#define TSD_ASM_VOLATILE volatile
+#else
+#define TSD_ASM_VOLATILE
+#endif
 #ifndef TSD_CONSTRAINED
 #define TSD_CONSTRAINED 0
 #endif
@@ -68,8 +84,20 @@ constexpr int STATE_BYTES = SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 con
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
 constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 8) * 4 + 15) / 16 * 16;   // bytes per chain
 constexpr u64 kObsLo = TSD_OBSMASK_LO, kObsHi = TSD_OBSMASK_HI;
-constexpr u32 kOnes = 0x01010101u, kTwos = 0x02020202u;
+constexpr u32 kOnes = 0x01010101u, kTops = 0x80808080u;
+constexpr int kImmaOrder = TSD_IMMA_ORDER;     // issue order of a phase's IMMAs: 0 word by word, 1 two words interleaved, 2 all words interleaved
+constexpr int RPT = SP ? (KS / 2) * 4 : KS * 4; // A-fragment registers per row tile
 constexpr bool kByteMism = NOBS * 2 * NW <= 255;   // mismatch counters stay in byte lanes
+// is time step t (1 .. T) scored?
+__host__ __device__ constexpr bool obs_at(int t) { return t < 64 ? ((kObsLo >> t) & 1ull) != 0ull : ((kObsHi >> (t - 64)) & 1ull) != 0ull; }
+// scored steps among 1 .. j-1
+__host__ __device__ constexpr int obs_before(int j) { int n = 0; for (int t = 1; t < j; ++t) n += obs_at(t) ? 1 : 0; return n; }
+__host__ __device__ constexpr bool obs_periodic() {
+  if (T % kTUnroll != 0) return false;
+  for (int t = 1; t + kTUnroll <= T; ++t) if (obs_at(t) != obs_at(t + kTUnroll)) return false;
+  return true;
+}
+constexpr bool kObsPeriodic = obs_periodic();
 static_assert(KS == 1 || KS == 2 || KS == 4, "KS must be 1, 2 or 4");
 static_assert(!SP || KS % 2 == 0, "the sparse layout needs whole 64-column steps");
 static_assert(!SWZ || (KS == 4 && TSD_W == 1), "the swizzled exchange buffer is for 16-byte units of one warp");
@@ -96,23 +124,23 @@ __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u3
   out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
-// 0xFF in every byte whose bit 7 is set, else 0x00
-__device__ __forceinline__ u32 sign_mask(u32 x) {
+// (a >> 1) + b as one multiply-add (IMAD.HI: the FMA pipe has room, the ALU pipe does the logic operations)
+__device__ __forceinline__ u32 half_plus(u32 a, u32 b) {
   u32 r;
-  asm("prmt.b32 %0, %1, 0, 0xBA98;" : "=r"(r) : "r"(x));
+  asm("mad.hi.u32 %0, %1, 0x80000000, %2;" : "=r"(r) : "r"(a), "r"(b));
   return r;
 }
 
-// D (16 x 8, s32) += A (16 x 32, s8, row) * B (32 x 8, s8, col)
+// D (16 x 8, s32) += A (16 x 32, s8, row) * B (32 x 8, u8, col)
 __device__ __forceinline__ void imma(int (&c)[4], const u32* a, u32 b0, u32 b1) {
-  asm volatile("mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+  asm TSD_ASM_VOLATILE("mma.sync.aligned.m16n8k32.row.col.s32.s8.u8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
                : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
 }
 
-// D (16 x 8, s32) += A (16 x 64, s8, 2:4 sparse: 16 x 32 stored + selectors e) * B (64 x 8, s8, col)
+// D (16 x 8, s32) += A (16 x 64, s8, 2:4 sparse: 16 x 32 stored + selectors e) * B (64 x 8, u8, col)
 __device__ __forceinline__ void imma_sp(int (&c)[4], const u32* a, u32 b0, u32 b1, u32 b2, u32 b3, u32 e) {
-  asm volatile("mma.sp::ordered_metadata.sync.aligned.m16n8k64.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9,%10,%11}, {%0,%1,%2,%3}, %12, 0x0;"
+  asm TSD_ASM_VOLATILE("mma.sp::ordered_metadata.sync.aligned.m16n8k64.row.col.s32.s8.u8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9,%10,%11}, {%0,%1,%2,%3}, %12, 0x0;"
                : "+r"(c[0]), "+r"(c[1]), "+r"(c[2]), "+r"(c[3])
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "r"(b2), "r"(b3), "r"(e));
 }
@@ -175,38 +203,44 @@ struct Regs {
   u32 A[NA];        // the warp's rows of the weight matrix: A fragments of its tile (mi, s) at [(mi*KS + s)*4 .. +3]
   u32 M[NM];        // sparse layout: selector words of the warp's tiles (the same for every chain)
   u32 TA[WPW];      // per byte (one row of this thread group): 0x80 - t_lo, padding rows 0
-  u32 TD[WPW];      // minus, per byte: t_hi - t_lo + 1, padding rows 0
-  u32 fix[NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows)
+  u32 TB[WPW];      // TA minus, per byte: t_hi - t_lo + 1 (padding rows 0)
+  u32 fix[NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows): bit 31 valid, 0-23 shared address of the byte
+  u32 fixv[NFIX];   // the byte to store there, 64 * value
 };
 
-// One phase of a time step: the IMMAs of the row tiles behind result words [P*WPP, (P+1)*WPP) of this
-// warp, then pack four sums to a word on top of the biased thresholds, compare, encode 0 / 1 / 2 per
-// byte, score against the observation words (a4) and store.  Phases run one after the other, so only
-// 2*WPP accumulator tiles are live at a time (the register budget that decides warps per SM).
+// One phase of a time step: the IMMAs of the row-tile pairs behind result words [P*WPP, (P+1)*WPP) of this
+// warp -- word w is the pair (2w, 2w+1): the even tile takes the states s and weights +-1, the odd tile the
+// bytes 64*s and weights +-4, both into ONE accumulator, so that accumulator register c holds
+// sum(tile 2w, row g) + 256 * sum(tile 2w+1, row g) and register 2+c the same for row g+8 -- then the word
+// acc[c] + 65536 * acc[2+c] on top of the biased thresholds, the two sign tests, the byte 64*s' per row,
+// the score against the observation words (a4) and the store.  Phases run one after the other.
 template <int P>
 struct Phases {
-  static __device__ __forceinline__ void run(const Regs& r, const u32 (&b)[2 * KS], int n_tiles, bool is_obs, const u32* ow,
-                                             u32& cnt, bool store, u32 st, u32 st1, int ring_me, int ring_next) {
-    constexpr int W0 = P * WPP;
-    int acc[2 * WPP][4];
+  // IMMA number `step` (0 .. 2*KK-1) of word w's accumulator chain: KK sparse / dense column steps of the even
+  // tile on the plain states, then KK of the odd tile on the 64-fold states
+  template <int KK>
+  static __device__ __forceinline__ void one(const Regs& r, const u32 (&bh)[2 * KS], const u32 (&bl)[2 * KS], int n_tiles,
+                                             int (&acc)[4], int w, int step) {
+    const int tile = 2 * (P * WPP + w) + step / KK, s = step % KK;
+    if (!(TW * MTW <= MT || tile < n_tiles)) return;
+    const u32* bb = step / KK ? bh : bl;
+    if (SP) imma_sp(acc, &r.A[(tile * KSP + s) * 4], bb[4 * s], bb[4 * s + 1], bb[4 * s + 2], bb[4 * s + 3], r.M[SP ? tile * KSP + s : 0]);
+    else imma(acc, &r.A[(tile * KS + s) * 4], bb[2 * s], bb[2 * s + 1]);
+  }
+  static __device__ __forceinline__ void run(const Regs& r, const u32 (&bh)[2 * KS], const u32 (&bl)[2 * KS], int n_tiles, bool is_obs,
+                                             const u32* ow, u32& cnt, bool store, u32 st, u32 st1, int ring_me, int ring_next) {
+    constexpr int W0 = P * WPP, KK = SP ? KSP : KS, NSTEP = 2 * KK;
+    int acc[WPP][4];
     if (CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
 #pragma unroll
-    for (int m = 0; m < 2 * WPP; ++m) { acc[m][0] = 0; acc[m][1] = 0; acc[m][2] = 0; acc[m][3] = 0; }
-    if (SP) {
+    for (int w = 0; w < WPP; ++w) { acc[w][0] = 0; acc[w][1] = 0; acc[w][2] = 0; acc[w][3] = 0; }
+    constexpr int GRP = kImmaOrder == 0 ? 1 : kImmaOrder == 1 ? 2 : WPP;     // words whose chains are interleaved
 #pragma unroll
-      for (int s = 0; s < KSP; ++s)
+    for (int w0 = 0; w0 < WPP; w0 += GRP)
 #pragma unroll
-        for (int mi = 0; mi < 2 * WPP; ++mi)
-          if (TW * MTW <= MT || 2 * W0 + mi < n_tiles)
-            imma_sp(acc[mi], &r.A[((2 * W0 + mi) * KSP + s) * 4], b[4 * s], b[4 * s + 1], b[4 * s + 2], b[4 * s + 3],
-                    r.M[SP ? (2 * W0 + mi) * KSP + s : 0]);
-    } else {
+      for (int step = 0; step < NSTEP; ++step)
 #pragma unroll
-      for (int s = 0; s < KS; ++s)
-#pragma unroll
-        for (int mi = 0; mi < 2 * WPP; ++mi)
-          if (TW * MTW <= MT || 2 * W0 + mi < n_tiles) imma(acc[mi], &r.A[((2 * W0 + mi) * KS + s) * 4], b[2 * s], b[2 * s + 1]);
-    }
+        for (int w = w0; w < w0 + GRP && w < WPP; ++w) one<KK>(r, bh, bl, n_tiles, acc[w], w, step);
     if (CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
     u32 ov[2][WPP];                                      // observation words, in flight while the sums are packed
     if (TSD_EARLY_OBS && is_obs) {
@@ -220,31 +254,30 @@ struct Phases {
     for (int w = 0; w < WPP; ++w)
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
-        const u32 x = r.TA[W0 + w] + (u32)acc[2 * w][c] + ((u32)acc[2 * w][2 + c] << 8) + ((u32)acc[2 * w + 1][c] << 16) +
-                      ((u32)acc[2 * w + 1][2 + c] << 24);
-        const u32 ge = sign_mask(x);
-        const u32 gt = sign_mask(x + r.TD[W0 + w]);
-        ns[c][w] = ((ge ^ gt) & kOnes) | (gt & kTwos);
+        const u32 pk = (u32)acc[w][c] + ((u32)acc[w][2 + c] << 16);
+        const u32 x = pk + r.TA[W0 + w], y = pk + r.TB[W0 + w];      // bit 7 of a byte: [sum >= t_lo], [sum > t_hi]
+        ns[c][w] = half_plus((x ^ y) & kTops, y & kTops);            // 0x40 = exactly one of them (the first), 0x80 = both
       }
     if (is_obs) {
 #pragma unroll
       for (int c = 0; c < 2; ++c)
 #pragma unroll
         for (int w = 0; w < WPP; ++w) {
-          const u32 z = ns[c][w] ^ (TSD_EARLY_OBS ? ov[c][w] : __ldg(ow + c * NW + W0 + w));
-          cnt += (z | (z >> 1)) & kOnes;
+          const u32 z = ns[c][w] ^ (TSD_EARLY_OBS ? ov[c][w] : __ldg(ow + c * NW + W0 + w));    // bits 6 and 7 of every byte
+          cnt = __umulhi((z | (z + z)) & kTops, 1u << 25) + cnt;                     // + [byte != 0] = (bit 7 | bit 6) >> 7
         }
     }
     if (store) {
       sts_vec(st + W0 * 4, ns[0]);
       sts_vec(st1 + W0 * 4, ns[1]);
     }
-    Phases<P + 1>::run(r, b, n_tiles, is_obs, ow, cnt, store, st, st1, ring_me, ring_next);
+    Phases<P + 1>::run(r, bh, bl, n_tiles, is_obs, ow, cnt, store, st, st1, ring_me, ring_next);
   }
 };
 template <>
 struct Phases<PH> {
-  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], int, bool, const u32*, u32&, bool, u32, u32, int, int) {}
+  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], const u32 (&)[2 * KS], int, bool, const u32*, u32&, bool,
+                                             u32, u32, int, int) {}
 };
 
 // a3 + a4 for the parameters now in registers: returns the team's mismatch count.
@@ -280,31 +313,40 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
     for (int i = 0; i < 2 * KS; ++i) b[i] = __ldg(src + i);
   }
   u32 mis = 0u;
-  int oj = 0;
-#pragma unroll (kTUnroll)
-  for (int t = 1; t <= T; ++t) {
-    const bool is_obs = t < 64 ? ((kObsLo >> t) & 1ull) : ((kObsHi >> (t - 64)) & 1ull);
+  int oj_run = 0;
+  // blocks of kTUnroll time steps; when the observation times repeat with that period, which steps of a
+  // block are scored (and the index of their observation words) is known at compile time
+#pragma unroll 1
+  for (int tb = 0; tb < T; tb += kTUnroll)
+#pragma unroll
+  for (int j = 1; j <= kTUnroll; ++j) {
+    const int t = tb + j;
+    if (T % kTUnroll != 0 && t > T) break;
+    const bool is_obs = kObsPeriodic ? obs_at(j) : obs_at(t);
+    const int oj = kObsPeriodic ? tb / kTUnroll * obs_before(kTUnroll + 1) + obs_before(j) : oj_run;
     const u32* ow = p.obs_word + ((size_t)oj * 32 + lane) * (2 * NW) + ww * WPW;
-    const u32 boff = NBUF == 2 ? (u32)(t & 1) * STATE_BYTES : 0u;
+    const u32 boff = NBUF == 2 ? (u32)((kTUnroll % 2 == 0 ? j : t) & 1) * STATE_BYTES : 0u;
     u32 cnt = 0u;                                         // per byte at most 2*WPW <= 8
     if (TW == 1) __syncwarp();            // every lane has its B fragments out of the single buffer
-    Phases<0>::run(r, b, n_tiles, is_obs, ow, cnt, t < T, st_addr + boff, st_addr + st_delta + boff, ring_me, ring_next);
+    u32 bl[2 * KS];                       // the plain states 0 / 1 / 2 for the even tiles
+#pragma unroll
+    for (int i = 0; i < 2 * KS; ++i) bl[i] = b[i] >> 6;
+    // (the last step's states are exchanged like all others although nobody reads them: no test in the loop)
+    Phases<0>::run(r, b, bl, n_tiles, is_obs, ow, cnt, true, st_addr + boff, st_addr + st_delta + boff, ring_me, ring_next);
     if (is_obs) {
       if (kByteMism) mis += cnt; else mis += __dp4a(cnt, kOnes, 0u);
-      ++oj;
+      ++oj_run;
     }
-    if (t < T) {
-      __syncwarp();
+    __syncwarp();
 #pragma unroll
-      for (int f = 0; f < NFIX; ++f)
-        if (r.fix[f] >> 31) sts_u8((r.fix[f] & 0xFFFFFFu) + boff, (r.fix[f] >> 24) & 3u);
-      team_sync();
-      u32 lo[NW], hi[NW];
-      lds_vec(ld_addr + boff, lo);
-      lds_vec(ld_addr + boff + (SWZ ? 512 : NW * 4), hi);
+    for (int f = 0; f < NFIX; ++f)
+      if (r.fix[f] >> 31) sts_u8((r.fix[f] & 0xFFFFFFu) + boff, r.fixv[f]);
+    team_sync();
+    u32 lo[NW], hi[NW];
+    lds_vec(ld_addr + boff, lo);
+    lds_vec(ld_addr + boff + (SWZ ? 512 : NW * 4), hi);
 #pragma unroll
-      for (int i = 0; i < NW; ++i) { b[i] = lo[i]; b[NW + i] = hi[i]; }
-    }
+    for (int i = 0; i < NW; ++i) { b[i] = lo[i]; b[NW + i] = hi[i]; }
   }
   u32 m = kByteMism ? __dp4a(mis, kOnes, 0u) : mis;
   m = __reduce_add_sync(0xffffffffu, m);
@@ -372,7 +414,8 @@ __device__ __forceinline__ Proposal propose(const Params& p, u64 gs, u32 gchain,
       if (TSD_CONSTRAINED) q.newv = constrained_weight(p, cw, q.pidx, q.oldv, x[1], &q.moved);
       else q.newv = (q.oldv + 2 + (int)__umulhi(x[1], 2u)) % 3 - 1;      // (code + 1 + r) mod 3 - 1, code = old + 1
       q.wsel = (int)(q.loc & 0x7Fu);
-      q.wx = ((u32)(q.oldv ^ q.newv) & 0xFFu) << (8 * ((q.loc >> 7) & 3u));
+      // the byte holds w (even row tiles) or 4w (odd ones)
+      q.wx = (((u32)(q.oldv ^ q.newv) << (((u32)q.wsel / (u32)RPT & 1u) * 2u)) & 0xFFu) << (8 * ((q.loc >> 7) & 3u));
     }
   } else {
     q.mine = (q.loc & 7u) == (u32)g && (int)((q.loc >> 3) & 3u) / WPW == ww;
@@ -390,7 +433,7 @@ __device__ __forceinline__ void shift_threshold(const Params& p, Regs& r, u32 lo
   const u32 da = (u32)((int)p.tha[to] - (int)p.tha[from]) << sh;
   const u32 dd = (u32)(((int)p.tha[from] - (int)p.thb[from]) - ((int)p.tha[to] - (int)p.thb[to])) << sh;
 #pragma unroll
-  for (int i = 0; i < WPW; ++i) if (i == w) { r.TA[i] += da; r.TD[i] += dd; }
+  for (int i = 0; i < WPW; ++i) if (i == w) { r.TA[i] += da; r.TB[i] += da + dd; }
 }
 
 __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int ring_me, int ring_next);
@@ -492,7 +535,8 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     const u32 b1 = o1 == 0xFFFFu ? 0u : (u32)(unsigned char)cw[o1];
     const u32 b2 = o2 == 0xFFFFu ? 0u : (u32)(unsigned char)cw[o2];
     const u32 b3 = o3 == 0xFFFFu ? 0u : (u32)(unsigned char)cw[o3];
-    r.A[i] = b0 | (b1 << 8) | (b2 << 16) | (b3 << 24);
+    const u32 wv = b0 | (b1 << 8) | (b2 << 16) | (b3 << 24);
+    r.A[i] = (i / RPT) & 1 ? (wv << 2) & 0xFCFCFCFCu : wv;       // odd row tiles hold 4w
   }
 #pragma unroll
   for (int i = 0; i < NM; ++i) r.M[i] = SP ? __ldg(p.meta + (ww * NM + i) * 32 + lane) : 0u;
@@ -508,12 +552,13 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
         td -= (u32)((int)p.tha[q] - (int)p.thb[q]) << (8 * j);
       }
     }
-    r.TA[w] = ta; r.TD[w] = td;
+    r.TA[w] = ta; r.TB[w] = ta + td;
   }
 #pragma unroll
-  for (int f = 0; f < NFIX; ++f) {                      // bit 31 valid, 24-25 value, 0-23 shared address of the byte
+  for (int f = 0; f < NFIX; ++f) {
     const u32 raw = __ldg(p.fix + (ww * NFIX + f) * 32 + lane);
-    r.fix[f] = (raw & 0x80000000u) | (((raw >> 16) & 3u) << 24) | (sbuf + (raw & 0xFFFFu));
+    r.fix[f] = (raw & 0x80000000u) | (sbuf + (raw & 0xFFFFu));
+    r.fixv[f] = ((raw >> 16) & 3u) << 6;
   }
 
   // Chain control words live in shared memory and the proposal is derived a second time after the

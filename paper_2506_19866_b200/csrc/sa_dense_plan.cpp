@@ -7,6 +7,8 @@ namespace tsa {
 
 namespace {
 
+constexpr uint32_t kStateScale = 64;   // the dense kernel exchanges a state s as the byte 64 * s (sa_dense_kernel.cu)
+
 // Shared-memory wavefronts of one warp-wide vector access (hardware serves 128 bytes per wavefront:
 // a quarter-warp of 16-byte accesses, a half-warp of 8-byte ones, the whole warp of 4-byte ones).
 int wavefronts(const int (&addr)[32], int vec_bytes) {
@@ -54,8 +56,9 @@ void pick_strides(int KS, int W, int* CS, int* TS, int* wf) {
   *wf = best;
 }
 
-// Node -> row assignment for the 2:4-sparse layout.  Four consecutive matrix columns are the rows
-// {32w + g + 8j : j = 0..3} (see col_of_row below); a row of W may hold at most two candidate
+// Node -> row assignment for the 2:4-sparse layout.  Four consecutive matrix columns are the four rows
+// that make up one result word of one thread group, {32w + g + 8x : x = 0..3} (see col_of_row below); a
+// row of W may hold at most two candidate
 // edges in any such group.  Local search over swaps and moves (deterministic), starting from the
 // identity; returns false if some violation is left.
 bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::vector<std::vector<int>>& out_dst,
@@ -120,14 +123,17 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   dp->swizzle = want_swizzle && KS == 4 && W == 1;
   if (dp->swizzle) dp->exchange_wavefronts = 16;
 
-  // Row r = 16m + 8h + g is produced by thread group g as byte j of its word w, q = 2m + h = 4w + j.
+  // Row r = 16m + 8h + g (row tile m, half h) is produced by thread group g.  The tiles 2w and 2w+1 share one
+  // accumulator (the odd tile's sums arrive 256-fold), whose registers c / 2+c are the halves h = 0 / 1, and the
+  // word is acc[c] + 65536 * acc[2+c]: so the row is byte j = 2h + (m & 1) of word w = m / 2.
   // That byte is stored at chunk t' = g % 4, word pos = (g / 4) * NW + w, which B-fragment thread t'
   // reads as column k = 16*pos + 4t' + j.
   auto col_of_row = [&](int r) {
-    const int m = r / 16, h = (r % 16) / 8, g = r % 8, q = 2 * m + h, w = q / 4, j = q % 4;
+    const int m = r / 16, h = (r % 16) / 8, g = r % 8, w = m / 2, j = 2 * h + (m & 1);
     const int pos = (g / 4) * NW + w;
     return 16 * pos + 4 * (g % 4) + j;
   };
+  auto row_of_byte = [&](int g, int w, int j) { return 16 * (2 * w + (j & 1)) + 8 * (j >> 1) + g; };
   // node -> row: the identity, or (sparse layout) a permutation that puts at most two of any node's
   // sources into the same group of four columns
   std::vector<int> row_of_node(N);
@@ -204,26 +210,27 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
               if (e1 >= 0) place(e1, m, wreg, lane, 2 * (G % 2) + 1, tile * 4 + a);
             }
   }
-  // thresholds: byte j of word w of thread group g <-> row 32w + 8j + g
+  // thresholds: byte j of word w of thread group g <-> row_of_byte(g, w, j)
   dp->th_entry.assign((size_t)8 * NW * 4, 0xFFFFu);
   dp->thloc.assign(N, 0u);
   for (int g = 0; g < 8; ++g)
     for (int w = 0; w < NW; ++w)
       for (int j = 0; j < 4; ++j) {
-        const int row = 32 * w + 8 * j + g;
+        const int row = row_of_byte(g, w, j);
         if (row >= 16 * MT || node_of_row[row] < 0) continue;
         const int node = node_of_row[row], entry = pl.entry_of_node[node];
         dp->th_entry[((size_t)g * NW + w) * 4 + j] = (uint16_t)entry;
         dp->thloc[node] = (uint32_t)g | ((uint32_t)w << 3) | ((uint32_t)j << 5) | ((uint32_t)entry << 16);
       }
-  // t = 0 states as B fragments: lane (g', t') word pos = columns 16 pos + 4t' + 0..3 of condition g'
+  // t = 0 states (as the bytes 64 * s, like every state the kernel exchanges) as B fragments: lane (g', t') word
+  // pos = columns 16 pos + 4t' + 0..3 of condition g'
   dp->init_frag.assign((size_t)32 * 2 * KS, 0u);
   for (int lane = 0; lane < 32; ++lane)
     for (int x = 0; x < 2 * KS; ++x)
       for (int j = 0; j < 4; ++j) {
         const int cond = lane / 4, col = 16 * x + 4 * (lane % 4) + j;
         if (cond >= K || node_of_col[col] < 0) continue;
-        dp->init_frag[(size_t)lane * 2 * KS + x] |= (uint32_t)obs->init_state[(size_t)cond * N + node_of_col[col]] << (8 * j);
+        dp->init_frag[(size_t)lane * 2 * KS + x] |= ((uint32_t)obs->init_state[(size_t)cond * N + node_of_col[col]] * kStateScale) << (8 * j);
       }
   // clamped (condition, node): restored by a byte store after every exchange; scored once, here
   // (the warp that owns the row's result word stores it, right after its own vector stores)
@@ -238,9 +245,9 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   for (int ww = 0; ww < W; ++ww) dp->n_fix_rounds = std::max(dp->n_fix_rounds, (int)(fixes[ww].size() + 31) / 32);
   dp->fix.assign((size_t)W * dp->n_fix_rounds * 32, 0u);
   for (int ww = 0; ww < W; ++ww) std::copy(fixes[ww].begin(), fixes[ww].end(), dp->fix.begin() + (size_t)ww * dp->n_fix_rounds * 32);
-  // observations in the layout of a lane's result words; 3 = never equal to a state, so such an
-  // entry always counts one mismatch, which fit_const takes back
-  dp->obs_word.assign((size_t)NO * 32 * 2 * NW, 0x03030303u);
+  // observations in the layout of a lane's result words, as the bytes 64 * value; 3 = never equal to a state, so
+  // such an entry always counts one mismatch, which fit_const takes back
+  dp->obs_word.assign((size_t)NO * 32 * 2 * NW, 0x01010101u * (3u * kStateScale));
   long always = (long)NO * 32 * 2 * NW * 4, clamped_mis = 0;
   if (obs->obs) {
     for (int oj = 0; oj < NO; ++oj)
@@ -248,7 +255,7 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
         for (int c = 0; c < 2; ++c)
           for (int w = 0; w < NW; ++w)
             for (int j = 0; j < 4; ++j) {
-              const int g = lane / 4, t = lane % 4, cond = 2 * t + c, row = 32 * w + 8 * j + g;
+              const int g = lane / 4, t = lane % 4, cond = 2 * t + c, row = row_of_byte(g, w, j);
               if (row >= 16 * MT || node_of_row[row] < 0 || cond >= K) continue;
               const int node = node_of_row[row];
               const uint8_t o = obs->obs[((size_t)cond * NO + oj) * N + node];
@@ -258,7 +265,7 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
                 continue;
               }
               uint32_t& word = dp->obs_word[((size_t)oj * 32 + lane) * 2 * NW + c * NW + w];
-              word = (word & ~(0xFFu << (8 * j))) | ((uint32_t)o << (8 * j));
+              word = (word & ~(0xFFu << (8 * j))) | (((uint32_t)o * kStateScale) << (8 * j));
               --always;
             }
   }
