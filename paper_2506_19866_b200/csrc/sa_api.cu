@@ -303,7 +303,7 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
   }
   tsa::build_dense_plan(net, obs, h->plan, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0,
-                        tsa::StaticTuning::from_env().dense_swizzle != 0, &h->dplan);
+                        tsa::StaticTuning::from_env().dense_swizzle != 0, tsa::StaticTuning::from_env().dense_movm != 0, &h->dplan);
   if (h->dplan.ok) {
     if ((rc = h->pool.upload(h->dplan.frag_slot, &h->d_frag_slot, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.th_entry, &h->d_th_entry, st))) return rc;
@@ -402,14 +402,15 @@ int sa_run(sa_handle* h, int64_t steps) {
     unsigned grid = (unsigned)((h->C.R + h->dk->chains_per_cta - 1) / h->dk->chains_per_cta);
     // More chains than resident slots: split the line of R*steps chain-steps evenly over the slots
     // (DESIGN.md §6 "balanced slots") instead of running ceil(R / slots) uneven waves.
-    const int64_t slots = (int64_t)h->dk->blocks_per_sm * h->sm_count;
+    const int cpb = h->dk->chains_per_cta;
+    const int64_t slots = (int64_t)h->dk->blocks_per_sm * h->sm_count * cpb;
     h->last_slot_steps = 0;
-    if (h->dk->chains_per_cta == 1 && slots > 0 && h->C.R > slots && !tsa::tune_env("TSA_DENSE_NO_BALANCE")) {
+    if (h->dk->free_slots && slots > 0 && h->C.R > slots && !tsa::tune_env("TSA_DENSE_NO_BALANCE")) {
       const int64_t total = (int64_t)h->C.R * steps;
       q.slot_steps = std::max<int64_t>((total + slots - 1) / slots, steps);
       q.flags = h->d_flags;
       TSA_CUDA(cudaMemsetAsync(h->d_flags, 0, (size_t)h->C.R * 4, h->stream));
-      grid = (unsigned)((total + q.slot_steps - 1) / q.slot_steps);
+      grid = (unsigned)(((total + q.slot_steps - 1) / q.slot_steps + cpb - 1) / cpb);
       h->last_slot_steps = q.slot_steps;
     }
     // A slot that holds the tail of a chain waits for the slot that holds its head, so every slot must
@@ -421,7 +422,7 @@ int sa_run(sa_handle* h, int64_t steps) {
       if (!launched) {
         q.slot_steps = 0; q.flags = nullptr;
         h->last_slot_steps = 0;
-        grid = (unsigned)h->C.R;
+        grid = (unsigned)((h->C.R + cpb - 1) / cpb);
       }
     }
     if (!launched && tsa::dense_kernel_launch(h->dk, grid, (void*)h->stream, q, &why) != 0) return set_err(SA_ECUDA, why);
@@ -661,7 +662,7 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
   {
     tsa::DensePlan dp;
     tsa::build_dense_plan(net, obs, pl, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0,
-                          tsa::StaticTuning::from_env().dense_swizzle != 0, &dp);
+                          tsa::StaticTuning::from_env().dense_swizzle != 0, tsa::StaticTuning::from_env().dense_movm != 0, &dp);
     if (dp.ok) {
       info[6] = 1;
       std::string cubin, clog;

@@ -46,8 +46,26 @@
 #define TSD_REDERIVE 1
 #define TSD_SP 1
 #define TSD_SWZ 1
-#define TSD_EARLY_OBS 0
+#define TSD_OBSW 2
 #define TSD_TUNROLL 1
+#define TSD_MOVM 1
+#define TSD_FIXW_MASK 1
+#endif
+#ifndef TSD_MOVM
+#define TSD_MOVM 0
+#endif
+#ifndef TSD_OBSW
+#define TSD_OBSW TSD_KS
+#endif
+#ifndef TSD_FIXW_MASK
+#define TSD_FIXW_MASK 0
+#endif
+#ifndef TSD_LOCK
+#define TSD_LOCK 0
+#endif
+
+#ifndef TSD_LOCK_REL
+#define TSD_LOCK_REL 3
 #endif
 #ifndef TSD_IMMA_ORDER
 #define TSD_IMMA_ORDER 0
@@ -80,14 +98,24 @@ constexpr int NA = SP ? MTW * KSP * 4 : MTW * KS * 4;   // A-fragment registers 
 constexpr int NM = SP ? MTW * KSP : 1;          // selector (metadata) registers per thread
 constexpr int kTUnroll = TSD_TUNROLL;           // unroll factor of the time loop
 constexpr bool SWZ = TSD_SWZ != 0;              // swizzled exchange buffer (KS = 4, one warp per chain): conflict-free stores AND loads
-constexpr int STATE_BYTES = SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 condition rows
+// Register exchange (v8): the result words reach the next step's B fragments through MOVM (movmatrix, an 8 x 8
+// transpose of 16-bit elements across the warp) instead of shared memory: no store, no barrier, no load.
+constexpr bool MOVM = TSD_MOVM != 0;
+constexpr u32 kFixW = TSD_FIXW_MASK;               // result words w that hold a clamped (condition, node) entry
+__host__ __device__ constexpr int popc_below(u32 m, int w) { int n = 0; for (int i = 0; i < w; ++i) n += (int)((m >> i) & 1u); return n; }
+constexpr int NFW = popc_below(kFixW, 32) > 0 ? popc_below(kFixW, 32) : 1;
+constexpr int STATE_BYTES = MOVM ? 0 : SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
 constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 8) * 4 + 15) / 16 * 16;   // bytes per chain
+// The host numbers the observed nodes first, so only the result words w < OBSW hold scored entries; the observation
+// words of a lane and time are stored w-major ([w][c]) and fetched with vector loads.
+constexpr int OBSW = TSD_OBSW;
+static_assert(OBSW >= 0 && OBSW <= NW, "scored words");
 constexpr u64 kObsLo = TSD_OBSMASK_LO, kObsHi = TSD_OBSMASK_HI;
 constexpr u32 kOnes = 0x01010101u, kTops = 0x80808080u;
 constexpr int kImmaOrder = TSD_IMMA_ORDER;     // issue order of a phase's IMMAs: 0 word by word, 1 two words interleaved, 2 all words interleaved
 constexpr int RPT = SP ? (KS / 2) * 4 : KS * 4; // A-fragment registers per row tile
-constexpr bool kByteMism = NOBS * 2 * NW <= 255;   // mismatch counters stay in byte lanes
+constexpr bool kByteMism = NOBS * 2 * (OBSW > 0 ? OBSW : 1) <= 255;   // mismatch counters stay in byte lanes
 // is time step t (1 .. T) scored?
 __host__ __device__ constexpr bool obs_at(int t) { return t < 64 ? ((kObsLo >> t) & 1ull) != 0ull : ((kObsHi >> (t - 64)) & 1ull) != 0ull; }
 // scored steps among 1 .. j-1
@@ -102,14 +130,26 @@ static_assert(KS == 1 || KS == 2 || KS == 4, "KS must be 1, 2 or 4");
 static_assert(!SP || KS % 2 == 0, "the sparse layout needs whole 64-column steps");
 static_assert(!SWZ || (KS == 4 && TSD_W == 1), "the swizzled exchange buffer is for 16-byte units of one warp");
 static_assert(2 * KS >= MT && MT >= 1, "row <-> column numbering needs MT <= 2*KS");
+static_assert(!MOVM || TSD_W == 1, "the register exchange is for one warp per chain");
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
 static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
-static_assert(CPB == 1 || (TW == 1 && CPB % 4 == 0 && CPB <= 16), "several chains per CTA: one-warp chains, whole rings, at most 15 named barriers");
+static_assert(CPB == 1 || (TW == 1 && (TSD_LOCK != 0 || CPB % 4 == 0) && CPB <= 16), "several chains per CTA: one-warp chains, whole rings, at most 15 named barriers");
 // CPB <= 12: one token per warp (a ring of CPB/4 warps per SM sub-partition, barrier 1 + warp).  CPB == 16: the four
 // warps of a sub-partition form two PAIRS that take turns on the tensor pipe (barriers 1 + 2q and 2 + 2q): while one
 // pair issues its 2 x 14 IMMAs the other pair does its integer work, which is what keeps both the pipe and the issue
 // port busy (free-running warps fall into lock step: all in the tensor phase, then all in the integer phase).
-constexpr bool kPairs = CPB == 16;
+// Tensor-pipe turn (v8, TSD_LOCK): the warps of one SM sub-partition share one tensor pipe, which serves the IMMAs
+// of all waiting warps in turn -- four warps that enter their tensor phase together leave it together, four
+// tensor phases later, and then do their integer work together while the pipe idles.  With one CTA of CPB
+// one-warp chains per SM, a warp enters its tensor phase only when the sub-partition's turn word in shared
+// memory is free and frees it when the accumulator of result word TSD_LOCK_REL is complete (the last IMMAs
+// are then in flight), so tensor phases follow one another and overlap the other warps' integer work.  The word
+// is a scheduling hint, taken with a plain load and store: two warps that take it at once just share the
+// pipe for that step, and nothing waits on a warp that is busy with its SA-step work (unlike the token ring).
+constexpr bool LOCK = TSD_LOCK != 0;
+constexpr int kLockRel = TSD_LOCK_REL;
+static_assert(!LOCK || (TW == 1 && PH == 1), "the tensor-pipe turn is for one-warp chains and one phase");
+constexpr bool kPairs = CPB == 16 && !LOCK;
 constexpr int kRingThreads = kPairs ? 128 : 64;
 
 // Philox4x32-10 (Salmon et al., SC'11)
@@ -128,6 +168,13 @@ __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u3
 __device__ __forceinline__ u32 half_plus(u32 a, u32 b) {
   u32 r;
   asm("mad.hi.u32 %0, %1, 0x80000000, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+// 8 x 8 transpose of 16-bit elements across the warp: lane (g, t) gives the elements (g, 2t), (g, 2t+1) and gets
+// (2t, g), (2t+1, g) (SASS MOVM.16.MT88)
+__device__ __forceinline__ u32 movm(u32 x) {
+  u32 r;
+  asm("movmatrix.sync.aligned.m8n8.trans.b16 %0, %1;" : "=r"(r) : "r"(x));
   return r;
 }
 
@@ -204,8 +251,10 @@ struct Regs {
   u32 M[NM];        // sparse layout: selector words of the warp's tiles (the same for every chain)
   u32 TA[WPW];      // per byte (one row of this thread group): 0x80 - t_lo, padding rows 0
   u32 TB[WPW];      // TA minus, per byte: t_hi - t_lo + 1 (padding rows 0)
-  u32 fix[NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows): bit 31 valid, 0-23 shared address of the byte
-  u32 fixv[NFIX];   // the byte to store there, 64 * value
+  u32 fix[MOVM ? 2 * NFW : NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows): bit 31 valid, 0-23 shared address of the byte
+  u32 fixv[MOVM ? 2 * NFW : NFIX];   // the byte to store there, 64 * value
+                    // register exchange: fix[2f + c] = bytes to keep, fixv[2f + c] = bytes 64 * value to set, of result word
+                    // (c, w) for the f-th w in kFixW
 };
 
 // One phase of a time step: the IMMAs of the row-tile pairs behind result words [P*WPP, (P+1)*WPP) of this
@@ -228,10 +277,11 @@ struct Phases {
     else imma(acc, &r.A[(tile * KS + s) * 4], bb[2 * s], bb[2 * s + 1]);
   }
   static __device__ __forceinline__ void run(const Regs& r, const u32 (&bh)[2 * KS], const u32 (&bl)[2 * KS], int n_tiles, bool is_obs,
-                                             const u32* ow, u32& cnt, bool store, u32 st, u32 st1, int ring_me, int ring_next) {
+                                             const u32 (&ov)[2 * WPW], int ww, u32& cnt, bool store, u32 st, u32 st1, int ring_me, int ring_next,
+                                             u32 (&nb)[2 * KS]) {
     constexpr int W0 = P * WPP, KK = SP ? KSP : KS, NSTEP = 2 * KK;
     int acc[WPP][4];
-    if (CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
+    if (!LOCK && CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
 #pragma unroll
     for (int w = 0; w < WPP; ++w) { acc[w][0] = 0; acc[w][1] = 0; acc[w][2] = 0; acc[w][3] = 0; }
     constexpr int GRP = kImmaOrder == 0 ? 1 : kImmaOrder == 1 ? 2 : WPP;     // words whose chains are interleaved
@@ -241,13 +291,11 @@ struct Phases {
       for (int step = 0; step < NSTEP; ++step)
 #pragma unroll
         for (int w = w0; w < w0 + GRP && w < WPP; ++w) one<KK>(r, bh, bl, n_tiles, acc[w], w, step);
-    if (CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
-    u32 ov[2][WPP];                                      // observation words, in flight while the sums are packed
-    if (TSD_EARLY_OBS && is_obs) {
-#pragma unroll
-      for (int c = 0; c < 2; ++c)
-#pragma unroll
-        for (int w = 0; w < WPP; ++w) ov[c][w] = __ldg(ow + c * NW + W0 + w);
+    if (!LOCK && CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
+    if (LOCK) {
+      // free the turn word once this accumulator is complete: the store's value depends on it (ring_next = the 0 read when the turn was taken)
+      const u32 z = (u32)acc[kLockRel < WPP ? kLockRel : WPP - 1][0] & (u32)ring_next;
+      asm volatile("st.shared.u32 [%0], %1;" ::"r"((u32)ring_me), "r"(z) : "memory");
     }
     u32 ns[2][WPP];
 #pragma unroll
@@ -263,21 +311,39 @@ struct Phases {
       for (int c = 0; c < 2; ++c)
 #pragma unroll
         for (int w = 0; w < WPP; ++w) {
-          const u32 z = ns[c][w] ^ (TSD_EARLY_OBS ? ov[c][w] : __ldg(ow + c * NW + W0 + w));    // bits 6 and 7 of every byte
+          if (TW == 1 ? W0 + w >= OBSW : ww * WPW + W0 + w >= OBSW) continue;      // no scored entry in this word
+          const u32 z = ns[c][w] ^ ov[2 * (W0 + w) + c];                             // bits 6 and 7 of every byte
           cnt = __umulhi((z | (z + z)) & kTops, 1u << 25) + cnt;                     // + [byte != 0] = (bit 7 | bit 6) >> 7
         }
     }
-    if (store) {
+    if (MOVM) {
+      // Word (c, w) of lane (g, t) holds rows g, g+8 of the tiles 2w, 2w+1 (bytes: 2w/g, 2w+1/g, 2w/g+8, 2w+1/g+8)
+      // under condition 2t + c.  The low halves of the words c = 0, 1 side by side are the elements (g, 2t), (g, 2t+1)
+      // of an 8 x 8 matrix [thread group][condition] of row pairs; its transpose gives lane (g', t') the pairs of
+      // the thread groups 2t', 2t'+1 under condition g': B-fragment word 2w of that lane (the high halves: word
+      // 2w+1) in the column numbering of sa_dense_plan.cpp.  Clamped entries are set before they travel.
+#pragma unroll
+      for (int w = 0; w < WPP; ++w) {
+        u32 n0 = ns[0][w], n1 = ns[1][w];
+        if ((kFixW >> (W0 + w)) & 1u) {
+          const int f = popc_below(kFixW, W0 + w);
+          n0 = (n0 & r.fix[2 * f]) | r.fixv[2 * f];
+          n1 = (n1 & r.fix[2 * f + 1]) | r.fixv[2 * f + 1];
+        }
+        nb[2 * (W0 + w)] = movm(__byte_perm(n0, n1, 0x5410));
+        nb[2 * (W0 + w) + 1] = movm(__byte_perm(n0, n1, 0x7632));
+      }
+    } else if (store) {
       sts_vec(st + W0 * 4, ns[0]);
       sts_vec(st1 + W0 * 4, ns[1]);
     }
-    Phases<P + 1>::run(r, bh, bl, n_tiles, is_obs, ow, cnt, store, st, st1, ring_me, ring_next);
+    Phases<P + 1>::run(r, bh, bl, n_tiles, is_obs, ov, ww, cnt, store, st, st1, ring_me, ring_next, nb);
   }
 };
 template <>
 struct Phases<PH> {
-  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], const u32 (&)[2 * KS], int, bool, const u32*, u32&, bool,
-                                             u32, u32, int, int) {}
+  static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], const u32 (&)[2 * KS], int, bool, const u32 (&)[2 * WPW], int, u32&,
+                                             bool, u32, u32, int, int, u32 (&)[2 * KS]) {}
 };
 
 // a3 + a4 for the parameters now in registers: returns the team's mismatch count.
@@ -291,8 +357,9 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
   // 4*(t'&1) + (c/2 + 2*(t'/2) + (c&1)) mod 4 -- a Latin square, so that the eight lanes of a quarter
   // warp hit eight different columns both when they store (c/2 and t'&1 vary) and when they load
   // (c&1, t'/2 and t'&1 vary).
-  u32 st_addr, st_delta, ld_addr;
-  if (SWZ) {
+  u32 st_addr = 0u, st_delta = 0u, ld_addr = 0u;
+  if (MOVM) {
+  } else if (SWZ) {
     const int tq = g & 3, half = g >> 2;
     const int q0 = 4 * (tq & 1) + ((t4 + 2 * (tq >> 1)) & 3), q1 = 4 * (tq & 1) + ((t4 + 2 * (tq >> 1) + 1) & 3);
     st_addr = sbuf + (u32)((4 * half + t4) * 128 + q0 * 16);
@@ -303,8 +370,8 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
     st_delta = (u32)CS;
     ld_addr = sbuf + (u32)(g * CS + t4 * TS);
   }
-  asm volatile("" : "+r"(st_addr), "+r"(ld_addr));      // keep them in registers (no S2R in the loop)
-  if (SWZ) asm volatile("" : "+r"(st_delta));
+  if (!MOVM) asm volatile("" : "+r"(st_addr), "+r"(ld_addr));      // keep them in registers (no S2R in the loop)
+  if (!MOVM && SWZ) asm volatile("" : "+r"(st_delta));
   const int n_tiles = MT - ww * MTW;                      // row tiles of this warp that exist (warp-uniform)
   u32 b[2 * KS];
   {
@@ -324,18 +391,56 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
     if (T % kTUnroll != 0 && t > T) break;
     const bool is_obs = kObsPeriodic ? obs_at(j) : obs_at(t);
     const int oj = kObsPeriodic ? tb / kTUnroll * obs_before(kTUnroll + 1) + obs_before(j) : oj_run;
-    const u32* ow = p.obs_word + ((size_t)oj * 32 + lane) * (2 * NW) + ww * WPW;
+    // observation words of this lane and time: [w][c], this warp's words first at 2 * ww * WPW
+    const u32* ow = p.obs_word + ((size_t)oj * 32 + lane) * (2 * NW) + 2 * ww * WPW;
+    u32 ov[2 * WPW];
+    if (is_obs) {
+      if (TW == 1) {
+        constexpr int VW = 2 * NW >= 4 ? 4 : 2;                 // words per vector load (a lane's 2 * NW words are that aligned)
+#pragma unroll
+        for (int v = 0; v * VW < 2 * OBSW; ++v) {
+          if (VW == 4) {
+            const uint4 q = __ldg((const uint4*)ow + v);
+            ov[4 * v] = q.x; ov[4 * v + 1] = q.y; ov[4 * v + 2] = q.z; ov[4 * v + 3] = q.w;
+          } else {
+            const uint2 q = __ldg((const uint2*)ow + v);
+            ov[2 * v] = q.x; ov[2 * v + 1] = q.y;
+          }
+        }
+      } else {
+#pragma unroll
+        for (int i = 0; i < 2 * WPW; ++i) if (ww * WPW + i / 2 < OBSW) ov[i] = __ldg(ow + i);
+      }
+    }
     const u32 boff = NBUF == 2 ? (u32)((kTUnroll % 2 == 0 ? j : t) & 1) * STATE_BYTES : 0u;
     u32 cnt = 0u;                                         // per byte at most 2*WPW <= 8
-    if (TW == 1) __syncwarp();            // every lane has its B fragments out of the single buffer
+    if (TW == 1 && !MOVM) __syncwarp();   // every lane has its B fragments out of the single buffer
     u32 bl[2 * KS];                       // the plain states 0 / 1 / 2 for the even tiles
+    u32 tok = 0u;
+    if (LOCK) {
+      // take the sub-partition's tensor-pipe turn; the word read (0) is the high half of the shifts below, so
+      // that every IMMA of this step depends on it
+      do {
+        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(tok) : "r"((u32)ring_me) : "memory");
+      } while (tok != 0u);
+      asm volatile("st.shared.u32 [%0], %1;" ::"r"((u32)ring_me), "r"(1u) : "memory");
+#pragma unroll
+      for (int i = 0; i < 2 * KS; ++i) bl[i] = __funnelshift_r(b[i], tok, 6);
+    } else {
 #pragma unroll
     for (int i = 0; i < 2 * KS; ++i) bl[i] = b[i] >> 6;
+    }
     // (the last step's states are exchanged like all others although nobody reads them: no test in the loop)
-    Phases<0>::run(r, b, bl, n_tiles, is_obs, ow, cnt, true, st_addr + boff, st_addr + st_delta + boff, ring_me, ring_next);
+    u32 nb[2 * KS];
+    Phases<0>::run(r, b, bl, n_tiles, is_obs, ov, ww, cnt, true, st_addr + boff, st_addr + st_delta + boff, ring_me, LOCK ? (int)tok : ring_next, nb);
     if (is_obs) {
       if (kByteMism) mis += cnt; else mis += __dp4a(cnt, kOnes, 0u);
       ++oj_run;
+    }
+    if (MOVM) {
+#pragma unroll
+      for (int i = 0; i < 2 * KS; ++i) b[i] = nb[i];
+      continue;
     }
     __syncwarp();
 #pragma unroll
@@ -454,7 +559,14 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
   // token ring of the CPB/4 one-warp chains that share this warp's SM sub-partition (warp wc, wc+4, ...):
   // on only if every member has a chain; then all of them run the same number of time steps
   int ring_me = 0, ring_next = 0;
-  if (CPB > 1) {
+  __shared__ u32 turn_word[4];
+  if (LOCK) {
+    if (threadIdx.x < 4) turn_word[threadIdx.x] = 0u;
+    __syncthreads();
+    u32 wid;
+    asm volatile("mov.u32 %0, %%warpid;" : "=r"(wid));               // hardware warp slot: slot & 3 = SM sub-partition
+    ring_me = (int)(u32)__cvta_generic_to_shared(&turn_word[wid & 3u]);
+  } else if (CPB > 1) {
     const int q = wc & 3, pos = wc >> 2, G = CPB >= 4 ? CPB / 4 : 1;
     if (blockIdx.x * CPB + (u32)(q + 4 * (G - 1)) < (u32)p.R) {
       if (kPairs) {
@@ -470,6 +582,7 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
     }
     if (chain >= (u32)p.R) return;
   }
+  if (LOCK && p.slot_steps == 0 && chain >= (u32)p.R) return;
   u32* const smem = smem_all + (size_t)wc * (CHAIN_SMEM / 4);
   // one chain per slot (slot_steps == 0), or balanced slots: this slot owns [lo, hi) of the line of
   // R*steps chain-steps and visits the chains ca .. cb it touches, one piece each
@@ -554,11 +667,19 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     }
     r.TA[w] = ta; r.TB[w] = ta + td;
   }
+  if (MOVM) {
 #pragma unroll
-  for (int f = 0; f < NFIX; ++f) {
-    const u32 raw = __ldg(p.fix + (ww * NFIX + f) * 32 + lane);
-    r.fix[f] = (raw & 0x80000000u) | (sbuf + (raw & 0xFFFFu));
-    r.fixv[f] = ((raw >> 16) & 3u) << 6;
+    for (int f = 0; f < 2 * NFW; ++f) {
+      r.fix[f] = __ldg(p.fix + (2 * f) * 32 + lane);
+      r.fixv[f] = __ldg(p.fix + (2 * f + 1) * 32 + lane);
+    }
+  } else {
+#pragma unroll
+    for (int f = 0; f < NFIX; ++f) {
+      const u32 raw = __ldg(p.fix + (ww * NFIX + f) * 32 + lane);
+      r.fix[f] = (raw & 0x80000000u) | (sbuf + (raw & 0xFFFFu));
+      r.fixv[f] = ((raw >> 16) & 3u) << 6;
+    }
   }
 
   // Chain control words live in shared memory and the proposal is derived a second time after the

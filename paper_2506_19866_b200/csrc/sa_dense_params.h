@@ -22,7 +22,7 @@ struct Params {
   const u32* meta;        // [tiles][32] sparse layout: selector word of each A tile, per lane
   const u16* th_entry;    // [8][NW][4]        canonical threshold-row offset of the node in (group g, word w, byte j), 0xFFFF = padding row
   const u32* init_frag;   // [32][2*KS]        B fragments of the t = 0 states, per lane
-  const u32* obs_word;    // [NOBS][32][2*NW]  observed values in the layout of a lane's result words (3 = not scored)
+  const u32* obs_word;    // [NOBS][32][NW][2] observed values in the layout of a lane's result words (3 = not scored)
   const u32* fix;         // [NFIX_ROUNDS][32] clamp fix-ups: bits 0-15 byte offset in the state buffer, 16-17 value, bit 31 valid
   const u32* wloc;        // [E]
   const u32* thloc;       // [N]

@@ -61,13 +61,15 @@ void pick_strides(int KS, int W, int* CS, int* TS, int* wf) {
 // row of W may hold at most two candidate
 // edges in any such group.  Local search over swaps and moves (deterministic), starting from the
 // identity; returns false if some violation is left.
+// movm: the register exchange's column numbering (a group = the rows 32w + 8h + 2t + {0, 1, 16, 17}).  A node of
+// zone z stays in the rows below zone_end[z] (clamped and observed nodes are kept in the first result words).
 bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::vector<std::vector<int>>& out_dst,
-                      int n_rows, std::vector<int>* row_of_node) {
+                      int n_rows, bool movm, const std::vector<int>& zone, const int (&zone_end)[3], std::vector<int>* row_of_node) {
   const int N = (int)in_src.size();
   std::vector<int>& row = *row_of_node;
   std::vector<int> node_at(n_rows, -1);
   for (int i = 0; i < N; ++i) node_at[row[i]] = i;
-  auto group_of = [&](int r) { return (r / 32) * 8 + r % 8; };
+  auto group_of = [&](int r) { return movm ? (r / 32) * 8 + ((r % 16) / 8) * 4 + (r % 8) / 2 : (r / 32) * 8 + r % 8; };
   auto row_cost = [&](int i) {
     int cnt[64] = {0}, c = 0;
     for (int s : in_src[i]) if (++cnt[group_of(row[s])] > 2) ++c;
@@ -83,6 +85,7 @@ bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::ve
   for (long it = 0; cost > 0 && it < 400000; ++it) {
     const int a = rnd(N), r2 = rnd(n_rows), b = node_at[r2];
     if (r2 == row[a] || (b >= 0 && group_of(row[b]) == group_of(row[a]))) continue;
+    if (r2 >= zone_end[zone[a]] || (b >= 0 && row[a] >= zone_end[zone[b]])) continue;
     long before = 0, after = 0;
     for (int i : out_dst[a]) before += row_cost(i);
     if (b >= 0) for (int i : out_dst[b]) before += row_cost(i);
@@ -104,7 +107,7 @@ bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::ve
 }  // namespace
 
 void build_dense_plan(const sa_network* net, const sa_observations* obs, const Plan& pl, int team_warps, bool want_sparse,
-                      bool want_swizzle, DensePlan* dp) {
+                      bool want_swizzle, bool want_movm, DensePlan* dp) {
   *dp = DensePlan();
   const int N = pl.N, E = pl.E, K = pl.K, NO = pl.n_obs;
   if (N > 128) { dp->why = "more than 128 nodes"; return; }
@@ -120,16 +123,22 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   dp->MT = MT; dp->KS = KS; dp->W = W;
   pick_strides(KS, W, &dp->CS, &dp->TS, &dp->exchange_wavefronts);
   const int CS = dp->CS, TS = dp->TS;
-  dp->swizzle = want_swizzle && KS == 4 && W == 1;
+  dp->movm = want_movm && W == 1;
+  dp->swizzle = want_swizzle && KS == 4 && W == 1 && !dp->movm;
   if (dp->swizzle) dp->exchange_wavefronts = 16;
+  if (dp->movm) dp->exchange_wavefronts = 0;
 
   // Row r = 16m + 8h + g (row tile m, half h) is produced by thread group g.  The tiles 2w and 2w+1 share one
   // accumulator (the odd tile's sums arrive 256-fold), whose registers c / 2+c are the halves h = 0 / 1, and the
   // word is acc[c] + 65536 * acc[2+c]: so the row is byte j = 2h + (m & 1) of word w = m / 2.
   // That byte is stored at chunk t' = g % 4, word pos = (g / 4) * NW + w, which B-fragment thread t'
   // reads as column k = 16*pos + 4t' + j.
+  // Register exchange (movm): the low (h = 0) / high (h = 1) halves of the words (0, w), (1, w) travel through one
+  // 8 x 8 transpose each and arrive as B-fragment word 2w + h of lane (g', t'), whose bytes are the rows
+  // 16(2w + (j & 1)) + 8h + 2t' + (j >> 1): column k = 16(2w + h) + 4t' + j.
   auto col_of_row = [&](int r) {
     const int m = r / 16, h = (r % 16) / 8, g = r % 8, w = m / 2, j = 2 * h + (m & 1);
+    if (dp->movm) return 16 * (2 * w + h) + 4 * (g / 2) + (m & 1) + 2 * (g & 1);
     const int pos = (g / 4) * NW + w;
     return 16 * pos + 4 * (g % 4) + j;
   };
@@ -138,16 +147,37 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   // sources into the same group of four columns
   std::vector<int> row_of_node(N);
   for (int i = 0; i < N; ++i) row_of_node[i] = i;
+  // Zones: clamped nodes first (register exchange only: the result words that need a fix-up are then few), then the
+  // other observed nodes (only the first result words are scored), then the rest; 32 rows per result word.
+  std::vector<int> zone(N, 2);
+  int zone_end[3] = {0, 0, 16 * MT};
+  {
+    int n0 = 0, n1 = 0;
+    for (int i = 0; i < N; ++i) {
+      bool clamped = false, observed = false;
+      for (int k = 0; k < K; ++k) {
+        if (obs->clamp[(size_t)k * N + i]) { clamped = true; continue; }
+        if (obs->obs)
+          for (int oj = 0; oj < NO; ++oj) observed |= obs->obs[((size_t)k * NO + oj) * N + i] != SA_UNOBSERVED;
+      }
+      zone[i] = (clamped && dp->movm) ? 0 : observed ? 1 : 2;
+      n0 += zone[i] == 0; n1 += zone[i] == 1;
+    }
+    zone_end[0] = std::min(16 * MT, (n0 + 31) / 32 * 32);
+    zone_end[1] = std::min(16 * MT, (n0 + n1 + 31) / 32 * 32);
+    int next[3] = {0, n0, n0 + n1};
+    for (int i = 0; i < N; ++i) row_of_node[i] = next[zone[i]]++;
+  }
   if (want_sparse && KS % 2 == 0) {
     std::vector<std::vector<int>> in_src(N), out_dst(N);
     for (int e = 0; e < E; ++e) { in_src[net->edge_dst[e]].push_back(net->edge_src[e]); out_dst[net->edge_src[e]].push_back(net->edge_dst[e]); }
     std::vector<int> trial = row_of_node;
-    if (assign_rows_2of4(in_src, out_dst, 16 * MT, &trial)) { row_of_node = trial; dp->sparse = true; }
+    if (assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, &trial)) { row_of_node = trial; dp->sparse = true; }
   }
   const int KSP = KS / 2;                            // sparse steps of 64 columns
   std::vector<int> node_of_row(32 * KS, -1), node_of_col(32 * KS, -1);
   for (int i = 0; i < N; ++i) { node_of_row[row_of_node[i]] = i; node_of_col[col_of_row(row_of_node[i])] = i; }
-  auto state_offset = [&](int cond, int node) {     // byte of (cond, node) in the exchange buffer
+  auto state_offset = [&](int cond, int node) {     // byte of (cond, node) in the exchange buffer (shared-memory exchange only)
     const int k = col_of_row(row_of_node[node]), pos = k / 16, tq = (k % 16) / 4, j = k % 4;
     if (dp->swizzle)                                 // see the kernel: row 4*half + c/2, column from a Latin square
       return (4 * (pos / 4) + cond / 2) * 128 + (4 * (tq & 1) + ((cond / 2 + 2 * (tq / 2) + (cond & 1)) & 3)) * 16 + (pos % 4) * 4 + j;
@@ -234,21 +264,55 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
       }
   // clamped (condition, node): restored by a byte store after every exchange; scored once, here
   // (the warp that owns the row's result word stores it, right after its own vector stores)
-  std::vector<std::vector<uint32_t>> fixes(W);
-  for (int k = 0; k < K; ++k)
-    for (int i = 0; i < N; ++i)
-      if (obs->clamp[(size_t)k * N + i]) {
-        const int ww = (row_of_node[i] / 32) / WPW;
-        fixes[ww].push_back((uint32_t)state_offset(k, i) | ((uint32_t)obs->init_state[(size_t)k * N + i] << 16) | 0x80000000u);
-      }
-  dp->n_fix_rounds = 1;
-  for (int ww = 0; ww < W; ++ww) dp->n_fix_rounds = std::max(dp->n_fix_rounds, (int)(fixes[ww].size() + 31) / 32);
-  dp->fix.assign((size_t)W * dp->n_fix_rounds * 32, 0u);
-  for (int ww = 0; ww < W; ++ww) std::copy(fixes[ww].begin(), fixes[ww].end(), dp->fix.begin() + (size_t)ww * dp->n_fix_rounds * 32);
-  // observations in the layout of a lane's result words, as the bytes 64 * value; 3 = never equal to a state, so
-  // such an entry always counts one mismatch, which fit_const takes back
+  if (dp->movm) {
+    // register exchange: per result word w that holds a clamped entry (bit w of fix_words), per c = 0, 1 and lane:
+    // the bytes to keep and the bytes 64 * value to set, [(2f + c) * 2 + {keep, value}][32]
+    dp->fix_words = 0;
+    for (int k = 0; k < K; ++k)
+      for (int i = 0; i < N; ++i)
+        if (obs->clamp[(size_t)k * N + i]) dp->fix_words |= 1u << (row_of_node[i] / 32);
+    int fidx[8], nf = 0;
+    for (int w = 0; w < NW; ++w) fidx[w] = ((dp->fix_words >> w) & 1u) ? nf++ : -1;
+    dp->n_fix_rounds = std::max(1, nf);
+    dp->fix.assign((size_t)dp->n_fix_rounds * 4 * 32, 0u);
+    for (int f = 0; f < dp->n_fix_rounds; ++f)
+      for (int c = 0; c < 2; ++c)
+        for (int lane = 0; lane < 32; ++lane) dp->fix[((size_t)(2 * f + c) * 2) * 32 + lane] = 0xFFFFFFFFu;
+    for (int k = 0; k < K; ++k)
+      for (int i = 0; i < N; ++i)
+        if (obs->clamp[(size_t)k * N + i]) {
+          const int r = row_of_node[i], m = r / 16, w = m / 2, j = 2 * ((r % 16) / 8) + (m & 1), g = r % 8;
+          const int lane = 4 * g + k / 2, c = k & 1, f = fidx[w];
+          dp->fix[((size_t)(2 * f + c) * 2) * 32 + lane] &= ~(0xFFu << (8 * j));
+          dp->fix[((size_t)(2 * f + c) * 2 + 1) * 32 + lane] |= ((uint32_t)obs->init_state[(size_t)k * N + i] * kStateScale) << (8 * j);
+        }
+  } else {
+    std::vector<std::vector<uint32_t>> fixes(W);
+    for (int k = 0; k < K; ++k)
+      for (int i = 0; i < N; ++i)
+        if (obs->clamp[(size_t)k * N + i]) {
+          const int ww = (row_of_node[i] / 32) / WPW;
+          fixes[ww].push_back((uint32_t)state_offset(k, i) | ((uint32_t)obs->init_state[(size_t)k * N + i] << 16) | 0x80000000u);
+        }
+    dp->n_fix_rounds = 1;
+    for (int ww = 0; ww < W; ++ww) dp->n_fix_rounds = std::max(dp->n_fix_rounds, (int)(fixes[ww].size() + 31) / 32);
+    dp->fix.assign((size_t)W * dp->n_fix_rounds * 32, 0u);
+    for (int ww = 0; ww < W; ++ww) std::copy(fixes[ww].begin(), fixes[ww].end(), dp->fix.begin() + (size_t)ww * dp->n_fix_rounds * 32);
+  }
+  // observations in the layout of a lane's result words ([w][c] per lane and time), as the bytes 64 * value; 3 = never
+  // equal to a state, so such an entry always counts one mismatch, which fit_const takes back.  Only the words
+  // w < obs_words hold a scored entry; the kernel looks at no other.
+  dp->obs_words = 0;
+  if (obs->obs)
+    for (int i = 0; i < N; ++i) {
+      bool scored = false;
+      for (int k = 0; k < K; ++k)
+        for (int oj = 0; oj < NO; ++oj)
+          scored |= !obs->clamp[(size_t)k * N + i] && obs->obs[((size_t)k * NO + oj) * N + i] != SA_UNOBSERVED;
+      if (scored) dp->obs_words = std::max(dp->obs_words, row_of_node[i] / 32 + 1);
+    }
   dp->obs_word.assign((size_t)NO * 32 * 2 * NW, 0x01010101u * (3u * kStateScale));
-  long always = (long)NO * 32 * 2 * NW * 4, clamped_mis = 0;
+  long always = (long)NO * 32 * 2 * dp->obs_words * 4, clamped_mis = 0;
   if (obs->obs) {
     for (int oj = 0; oj < NO; ++oj)
       for (int lane = 0; lane < 32; ++lane)
@@ -264,7 +328,7 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
                 if (o != obs->init_state[(size_t)cond * N + node]) ++clamped_mis;
                 continue;
               }
-              uint32_t& word = dp->obs_word[((size_t)oj * 32 + lane) * 2 * NW + c * NW + w];
+              uint32_t& word = dp->obs_word[((size_t)oj * 32 + lane) * 2 * NW + 2 * w + c];
               word = (word & ~(0xFFu << (8 * j))) | (((uint32_t)o * kStateScale) << (8 * j));
               --always;
             }
