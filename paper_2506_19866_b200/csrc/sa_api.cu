@@ -162,11 +162,14 @@ bool use_dense(sa_handle* h) {
   if (!h->dk_tried) {
     h->dk_tried = true;
     tsa::StaticTuning tune = tsa::StaticTuning::from_env();
-    if (!tsa::tune_env("TSA_DENSE_BLOCKS")) {
-      // fewer chains than slots: do not squeeze the registers for an occupancy the grid cannot reach
-      const int per_sm = (int)((h->C.R + h->sm_count - 1) / std::max(h->sm_count, 1));
-      tune.dense_blocks = std::max(1, std::min(h->dplan.sparse ? 16 : 12, per_sm));
-    }
+    // chains per SM the registers allow (16 at 128 registers with the sparse operand, 12 at 168 with the dense one);
+    // fewer chains than that: do not squeeze the registers for an occupancy the grid cannot reach
+    const int per_sm = (int)((h->C.R + h->sm_count - 1) / std::max(h->sm_count, 1));
+    const int resident = std::max(1, std::min(h->dplan.sparse ? 16 : 12, per_sm));
+    if (!tsa::tune_env("TSA_DENSE_BLOCKS")) tune.dense_blocks = resident;
+    // one-warp chains: all of an SM's chains in ONE CTA, whose warps the hardware spreads evenly over the four
+    // sub-partitions (one-warp CTAs land unevenly: measured 155 against 163 M chain-steps/s on Mtb-shaped)
+    if (tune.dense_cpb == 0) tune.dense_cpb = h->dplan.W == 1 ? (tune.dense_blocks > 0 && tsa::tune_env("TSA_DENSE_BLOCKS") ? 1 : resident) : 1;
     tune.constrained = h->S.constrained ? 1 : 0;
     h->dk = tsa::dense_kernel_get(h->plan, h->dplan, tune, &h->dense_why);
   }
@@ -405,7 +408,7 @@ int sa_run(sa_handle* h, int64_t steps) {
     const int cpb = h->dk->chains_per_cta;
     const int64_t slots = (int64_t)h->dk->blocks_per_sm * h->sm_count * cpb;
     h->last_slot_steps = 0;
-    if (h->dk->free_slots && slots > 0 && h->C.R > slots && !tsa::tune_env("TSA_DENSE_NO_BALANCE")) {
+    if (slots > 0 && h->C.R > slots && !tsa::tune_env("TSA_DENSE_NO_BALANCE")) {
       const int64_t total = (int64_t)h->C.R * steps;
       q.slot_steps = std::max<int64_t>((total + slots - 1) / slots, steps);
       q.flags = h->d_flags;

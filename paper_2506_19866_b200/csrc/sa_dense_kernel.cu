@@ -57,15 +57,11 @@
 #ifndef TSD_OBSW
 #define TSD_OBSW TSD_KS
 #endif
+#ifndef TSD_CFOLD
+#define TSD_CFOLD 0
+#endif
 #ifndef TSD_FIXW_MASK
 #define TSD_FIXW_MASK 0
-#endif
-#ifndef TSD_LOCK
-#define TSD_LOCK 0
-#endif
-
-#ifndef TSD_LOCK_REL
-#define TSD_LOCK_REL 3
 #endif
 #ifndef TSD_IMMA_ORDER
 #define TSD_IMMA_ORDER 0
@@ -88,7 +84,13 @@ constexpr int MT = TSD_MT, KS = TSD_KS, NW = TSD_KS, T = TSD_T, NOBS = TSD_NOBS;
 constexpr int CS = TSD_CS, TS = TSD_TS, NFIX = TSD_NFIX;
 constexpr int TW = TSD_W, TEAM = TW * 32;       // warps / threads per chain
 constexpr bool REDERIVE = TSD_REDERIVE != 0;    // tight register budget: derive the proposal twice rather than hold it over the time loop
-constexpr int CPB = TSD_CPB;                    // chains per CTA (one-warp chains only): 4 token rings of CPB/4 warps
+// TSD_CFOLD: the biased thresholds 0x80 - t_lo enter as the C operand of the first IMMA of every accumulator (a quad
+// of registers per result word, the two halves of the word TA twice), so the packed word already is x and the add
+// of TA goes away.  An IMMA that reads a C quad instead of RZ costs more issue time than the add it saves on
+// Mtb-shaped (149 against 164 M chain-steps/s); it gains 2 % where a chain has two IMMAs per step (HPG-shaped).
+constexpr bool CFOLD = TSD_CFOLD != 0;
+constexpr int CPB = TSD_CPB;                    // chains per CTA (one-warp chains only), independent of one another: a CTA of
+                                                // 4k warps puts k chains on every SM sub-partition, which 4k one-warp CTAs do not
 constexpr int WPW = NW / TW;                    // result words per condition a lane produces
 constexpr int MTW = 2 * WPW;                    // row tiles per warp (the last warp's may lie beyond MT)
 constexpr int PH = TSD_PH, WPP = WPW / PH;       // phases of a time step, result words per phase
@@ -133,25 +135,7 @@ static_assert(2 * KS >= MT && MT >= 1, "row <-> column numbering needs MT <= 2*K
 static_assert(!MOVM || TSD_W == 1, "the register exchange is for one warp per chain");
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
 static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
-static_assert(CPB == 1 || (TW == 1 && (TSD_LOCK != 0 || CPB % 4 == 0) && CPB <= 16), "several chains per CTA: one-warp chains, whole rings, at most 15 named barriers");
-// CPB <= 12: one token per warp (a ring of CPB/4 warps per SM sub-partition, barrier 1 + warp).  CPB == 16: the four
-// warps of a sub-partition form two PAIRS that take turns on the tensor pipe (barriers 1 + 2q and 2 + 2q): while one
-// pair issues its 2 x 14 IMMAs the other pair does its integer work, which is what keeps both the pipe and the issue
-// port busy (free-running warps fall into lock step: all in the tensor phase, then all in the integer phase).
-// Tensor-pipe turn (v8, TSD_LOCK): the warps of one SM sub-partition share one tensor pipe, which serves the IMMAs
-// of all waiting warps in turn -- four warps that enter their tensor phase together leave it together, four
-// tensor phases later, and then do their integer work together while the pipe idles.  With one CTA of CPB
-// one-warp chains per SM, a warp enters its tensor phase only when the sub-partition's turn word in shared
-// memory is free and frees it when the accumulator of result word TSD_LOCK_REL is complete (the last IMMAs
-// are then in flight), so tensor phases follow one another and overlap the other warps' integer work.  The word
-// is a scheduling hint, taken with a plain load and store: two warps that take it at once just share the
-// pipe for that step, and nothing waits on a warp that is busy with its SA-step work (unlike the token ring).
-constexpr bool LOCK = TSD_LOCK != 0;
-constexpr int kLockRel = TSD_LOCK_REL;
-static_assert(!LOCK || (TW == 1 && PH == 1), "the tensor-pipe turn is for one-warp chains and one phase");
-constexpr bool kPairs = CPB == 16 && !LOCK;
-constexpr int kRingThreads = kPairs ? 128 : 64;
-
+static_assert(CPB == 1 || (TW == 1 && CPB <= 16), "several chains per CTA: one-warp chains");
 // Philox4x32-10 (Salmon et al., SC'11)
 __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1, u32 (&out)[4]) {
 #pragma unroll
@@ -192,6 +176,18 @@ __device__ __forceinline__ void imma_sp(int (&c)[4], const u32* a, u32 b0, u32 b
                : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "r"(b2), "r"(b3), "r"(e));
 }
 
+// the same with a separate C operand (the first IMMA of an accumulator chain under CFOLD)
+__device__ __forceinline__ void imma_c(int (&c)[4], const u32* a, u32 b0, u32 b1, const u32 (&ci)[4]) {
+  asm TSD_ASM_VOLATILE("mma.sync.aligned.m16n8k32.row.col.s32.s8.u8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%11,%12,%13};"
+               : "=r"(c[0]), "=r"(c[1]), "=r"(c[2]), "=r"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "r"(ci[0]), "r"(ci[1]), "r"(ci[2]), "r"(ci[3]));
+}
+__device__ __forceinline__ void imma_sp_c(int (&c)[4], const u32* a, u32 b0, u32 b1, u32 b2, u32 b3, u32 e, const u32 (&ci)[4]) {
+  asm TSD_ASM_VOLATILE("mma.sp::ordered_metadata.sync.aligned.m16n8k64.row.col.s32.s8.u8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9,%10,%11}, {%13,%14,%15,%16}, %12, 0x0;"
+               : "=r"(c[0]), "=r"(c[1]), "=r"(c[2]), "=r"(c[3])
+               : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1), "r"(b2), "r"(b3), "r"(e), "r"(ci[0]), "r"(ci[1]), "r"(ci[2]), "r"(ci[3]));
+}
+
 __device__ __forceinline__ void team_sync() {
   if (TW == 1) __syncwarp(); else __syncthreads();
 }
@@ -224,14 +220,6 @@ __device__ __forceinline__ void sts_vec(u32 a, const u32 (&s)[4]) {
 }
 __device__ __forceinline__ void sts_u8(u32 a, u32 v) { smem_check(a, 1); asm volatile("st.shared.u8 [%0], %1;" ::"r"(a), "r"(v) : "memory"); }
 
-// Tensor-pipe token ring.  Warps that share an SM sub-partition would otherwise fall into lock step
-// (all issue IMMAs together, then all do the integer work together, and the tensor pipe idles
-// half the time); instead the warp holding the token issues its IMMAs, passes the token on, and does
-// its integer work while the next warp uses the pipe.  One named barrier per warp, 64 threads:
-// the waiting warp's bar.sync and its predecessor's bar.arrive.
-__device__ __forceinline__ void ring_wait(int id) { asm volatile("bar.sync %0, %1;" ::"r"(id), "n"(kRingThreads) : "memory"); }
-__device__ __forceinline__ void ring_pass(int id) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "n"(kRingThreads) : "memory"); }
-
 // a[sel] ^= x for a run-time sel (a jump table: registers cannot be indexed); sel outside [0, NA) does nothing
 #define TSD_C1(i) case (i): if ((i) < NA) a[(i) < NA ? (i) : 0] ^= x; break;
 #define TSD_C4(i) TSD_C1(i) TSD_C1((i) + 1) TSD_C1((i) + 2) TSD_C1((i) + 3)
@@ -249,8 +237,9 @@ __device__ __forceinline__ void xor_reg(u32 (&a)[NA], int sel, u32 x) {
 struct Regs {
   u32 A[NA];        // the warp's rows of the weight matrix: A fragments of its tile (mi, s) at [(mi*KS + s)*4 .. +3]
   u32 M[NM];        // sparse layout: selector words of the warp's tiles (the same for every chain)
-  u32 TA[WPW];      // per byte (one row of this thread group): 0x80 - t_lo, padding rows 0
-  u32 TB[WPW];      // TA minus, per byte: t_hi - t_lo + 1 (padding rows 0)
+  u32 TA[CFOLD ? 1 : WPW];      // per byte (one row of this thread group): 0x80 - t_lo, padding rows 0
+  u32 TB[WPW];      // TA minus, per byte: t_hi - t_lo + 1 (padding rows 0); CFOLD: only that difference
+  u32 CI[CFOLD ? WPW : 1][4];   // CFOLD: TA & 0xFFFF twice, TA >> 16 twice
   u32 fix[MOVM ? 2 * NFW : NFIX];    // clamp fix-ups of this lane (entries of the warp's own rows): bit 31 valid, 0-23 shared address of the byte
   u32 fixv[MOVM ? 2 * NFW : NFIX];   // the byte to store there, 64 * value
                     // register exchange: fix[2f + c] = bytes to keep, fixv[2f + c] = bytes 64 * value to set, of result word
@@ -273,15 +262,18 @@ struct Phases {
     const int tile = 2 * (P * WPP + w) + step / KK, s = step % KK;
     if (!(TW * MTW <= MT || tile < n_tiles)) return;
     const u32* bb = step / KK ? bh : bl;
+    if (CFOLD && step == 0) {
+      if (SP) imma_sp_c(acc, &r.A[(tile * KSP + s) * 4], bb[4 * s], bb[4 * s + 1], bb[4 * s + 2], bb[4 * s + 3], r.M[SP ? tile * KSP + s : 0], r.CI[CFOLD ? P * WPP + w : 0]);
+      else imma_c(acc, &r.A[(tile * KS + s) * 4], bb[2 * s], bb[2 * s + 1], r.CI[CFOLD ? P * WPP + w : 0]);
+      return;
+    }
     if (SP) imma_sp(acc, &r.A[(tile * KSP + s) * 4], bb[4 * s], bb[4 * s + 1], bb[4 * s + 2], bb[4 * s + 3], r.M[SP ? tile * KSP + s : 0]);
     else imma(acc, &r.A[(tile * KS + s) * 4], bb[2 * s], bb[2 * s + 1]);
   }
   static __device__ __forceinline__ void run(const Regs& r, const u32 (&bh)[2 * KS], const u32 (&bl)[2 * KS], int n_tiles, bool is_obs,
-                                             const u32 (&ov)[2 * WPW], int ww, u32& cnt, bool store, u32 st, u32 st1, int ring_me, int ring_next,
-                                             u32 (&nb)[2 * KS]) {
+                                             const u32 (&ov)[2 * WPW], int ww, u32& cnt, bool store, u32 st, u32 st1, u32 (&nb)[2 * KS]) {
     constexpr int W0 = P * WPP, KK = SP ? KSP : KS, NSTEP = 2 * KK;
     int acc[WPP][4];
-    if (!LOCK && CPB > 1 && P == 0 && ring_me) ring_wait(ring_me);
 #pragma unroll
     for (int w = 0; w < WPP; ++w) { acc[w][0] = 0; acc[w][1] = 0; acc[w][2] = 0; acc[w][3] = 0; }
     constexpr int GRP = kImmaOrder == 0 ? 1 : kImmaOrder == 1 ? 2 : WPP;     // words whose chains are interleaved
@@ -291,19 +283,13 @@ struct Phases {
       for (int step = 0; step < NSTEP; ++step)
 #pragma unroll
         for (int w = w0; w < w0 + GRP && w < WPP; ++w) one<KK>(r, bh, bl, n_tiles, acc[w], w, step);
-    if (!LOCK && CPB > 1 && P == PH - 1 && ring_next) ring_pass(ring_next);
-    if (LOCK) {
-      // free the turn word once this accumulator is complete: the store's value depends on it (ring_next = the 0 read when the turn was taken)
-      const u32 z = (u32)acc[kLockRel < WPP ? kLockRel : WPP - 1][0] & (u32)ring_next;
-      asm volatile("st.shared.u32 [%0], %1;" ::"r"((u32)ring_me), "r"(z) : "memory");
-    }
     u32 ns[2][WPP];
 #pragma unroll
     for (int w = 0; w < WPP; ++w)
 #pragma unroll
       for (int c = 0; c < 2; ++c) {
         const u32 pk = (u32)acc[w][c] + ((u32)acc[w][2 + c] << 16);
-        const u32 x = pk + r.TA[W0 + w], y = pk + r.TB[W0 + w];      // bit 7 of a byte: [sum >= t_lo], [sum > t_hi]
+        const u32 x = CFOLD ? pk : pk + r.TA[CFOLD ? 0 : W0 + w], y = pk + r.TB[W0 + w];      // bit 7 of a byte: [sum >= t_lo], [sum > t_hi]
         ns[c][w] = half_plus((x ^ y) & kTops, y & kTops);            // 0x40 = exactly one of them (the first), 0x80 = both
       }
     if (is_obs) {
@@ -337,19 +323,18 @@ struct Phases {
       sts_vec(st + W0 * 4, ns[0]);
       sts_vec(st1 + W0 * 4, ns[1]);
     }
-    Phases<P + 1>::run(r, bh, bl, n_tiles, is_obs, ov, ww, cnt, store, st, st1, ring_me, ring_next, nb);
+    Phases<P + 1>::run(r, bh, bl, n_tiles, is_obs, ov, ww, cnt, store, st, st1, nb);
   }
 };
 template <>
 struct Phases<PH> {
   static __device__ __forceinline__ void run(const Regs&, const u32 (&)[2 * KS], const u32 (&)[2 * KS], int, bool, const u32 (&)[2 * WPW], int, u32&,
-                                             bool, u32, u32, int, int, u32 (&)[2 * KS]) {}
+                                             bool, u32, u32, u32 (&)[2 * KS]) {}
 };
 
 // a3 + a4 for the parameters now in registers: returns the team's mismatch count.
 // sbuf = shared address of the exchange buffer(s), red = the team's reduction words [2][TW].
-__device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf, volatile u32* red, int parity, int lane, int ww,
-                                        int ring_me, int ring_next) {
+__device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf, volatile u32* red, int parity, int lane, int ww) {
   const int g = lane >> 2, t4 = lane & 3;
   // Exchange buffer.  Plain layout: condition rows of CS bytes, thread chunks of TS bytes (strides from
   // the host's conflict search).  Swizzled layout (16-byte units, unit (c, t', half) = the words
@@ -416,23 +401,11 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Regs& r, u32 sbuf
     u32 cnt = 0u;                                         // per byte at most 2*WPW <= 8
     if (TW == 1 && !MOVM) __syncwarp();   // every lane has its B fragments out of the single buffer
     u32 bl[2 * KS];                       // the plain states 0 / 1 / 2 for the even tiles
-    u32 tok = 0u;
-    if (LOCK) {
-      // take the sub-partition's tensor-pipe turn; the word read (0) is the high half of the shifts below, so
-      // that every IMMA of this step depends on it
-      do {
-        asm volatile("ld.volatile.shared.u32 %0, [%1];" : "=r"(tok) : "r"((u32)ring_me) : "memory");
-      } while (tok != 0u);
-      asm volatile("st.shared.u32 [%0], %1;" ::"r"((u32)ring_me), "r"(1u) : "memory");
-#pragma unroll
-      for (int i = 0; i < 2 * KS; ++i) bl[i] = __funnelshift_r(b[i], tok, 6);
-    } else {
 #pragma unroll
     for (int i = 0; i < 2 * KS; ++i) bl[i] = b[i] >> 6;
-    }
     // (the last step's states are exchanged like all others although nobody reads them: no test in the loop)
     u32 nb[2 * KS];
-    Phases<0>::run(r, b, bl, n_tiles, is_obs, ov, ww, cnt, true, st_addr + boff, st_addr + st_delta + boff, ring_me, LOCK ? (int)tok : ring_next, nb);
+    Phases<0>::run(r, b, bl, n_tiles, is_obs, ov, ww, cnt, true, st_addr + boff, st_addr + st_delta + boff, nb);
     if (is_obs) {
       if (kByteMism) mis += cnt; else mis += __dp4a(cnt, kOnes, 0u);
       ++oj_run;
@@ -538,10 +511,20 @@ __device__ __forceinline__ void shift_threshold(const Params& p, Regs& r, u32 lo
   const u32 da = (u32)((int)p.tha[to] - (int)p.tha[from]) << sh;
   const u32 dd = (u32)(((int)p.tha[from] - (int)p.thb[from]) - ((int)p.tha[to] - (int)p.thb[to])) << sh;
 #pragma unroll
-  for (int i = 0; i < WPW; ++i) if (i == w) { r.TA[i] += da; r.TB[i] += da + dd; }
+  for (int i = 0; i < WPW; ++i)
+    if (i == w) {
+      if (CFOLD) {
+        const u32 ta = r.CI[CFOLD ? i : 0][0] + (r.CI[CFOLD ? i : 0][2] << 16) + da;
+        r.CI[CFOLD ? i : 0][0] = ta & 0xFFFFu; r.CI[CFOLD ? i : 0][1] = ta & 0xFFFFu;
+        r.CI[CFOLD ? i : 0][2] = ta >> 16; r.CI[CFOLD ? i : 0][3] = ta >> 16;
+        r.TB[i] += dd;
+      } else {
+        r.TA[CFOLD ? 0 : i] += da; r.TB[i] += da + dd;
+      }
+    }
 }
 
-__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int ring_me, int ring_next);
+__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix);
 
 // add the piece's counts of level ctl[6] to the handle's table and clear them (one thread per chain)
 __device__ __noinline__ void flush_stats(const Params& p, volatile u32* ctl) {
@@ -556,33 +539,7 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
   extern __shared__ __align__(16) u32 smem_all[];
   const int tix = threadIdx.x % TEAM, wc = threadIdx.x / TEAM;       // thread within the chain's team, chain slot within the CTA
   const u32 chain = blockIdx.x * CPB + wc;
-  // token ring of the CPB/4 one-warp chains that share this warp's SM sub-partition (warp wc, wc+4, ...):
-  // on only if every member has a chain; then all of them run the same number of time steps
-  int ring_me = 0, ring_next = 0;
-  __shared__ u32 turn_word[4];
-  if (LOCK) {
-    if (threadIdx.x < 4) turn_word[threadIdx.x] = 0u;
-    __syncthreads();
-    u32 wid;
-    asm volatile("mov.u32 %0, %%warpid;" : "=r"(wid));               // hardware warp slot: slot & 3 = SM sub-partition
-    ring_me = (int)(u32)__cvta_generic_to_shared(&turn_word[wid & 3u]);
-  } else if (CPB > 1) {
-    const int q = wc & 3, pos = wc >> 2, G = CPB >= 4 ? CPB / 4 : 1;
-    if (blockIdx.x * CPB + (u32)(q + 4 * (G - 1)) < (u32)p.R) {
-      if (kPairs) {
-        const int pair = pos >> 1;                                     // warps q, q+4 are pair 0; q+8, q+12 pair 1
-        ring_me = 1 + 2 * q + pair;
-        ring_next = 1 + 2 * q + (1 - pair);
-        if (pair == 1) ring_pass(ring_next);                           // pair 0 goes first
-      } else {
-        ring_me = 1 + wc;
-        ring_next = 1 + q + 4 * ((pos + 1) % G);
-        if (pos == G - 1) ring_pass(ring_next);                        // the token starts at the ring's first warp
-      }
-    }
-    if (chain >= (u32)p.R) return;
-  }
-  if (LOCK && p.slot_steps == 0 && chain >= (u32)p.R) return;
+  if (p.slot_steps == 0 && chain >= (u32)p.R) return;
   u32* const smem = smem_all + (size_t)wc * (CHAIN_SMEM / 4);
   // one chain per slot (slot_steps == 0), or balanced slots: this slot owns [lo, hi) of the line of
   // R*steps chain-steps and visits the chains ca .. cb it touches, one piece each
@@ -602,7 +559,7 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
     const bool head_first = cb > ca && hi < (cb + 1) * S;
     const i64 c = n == count - 1 ? ca : head_first ? (n == 0 ? cb : ca + n) : ca + 1 + n;
     const i64 b0 = c * S;
-    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix, ring_me, ring_next);
+    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix);
   }
 }
 
@@ -611,7 +568,7 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
 // are more chains than resident slots the host splits the (chain, step) line evenly over the slots
 // (slot_steps > 0), and a chain that straddles two slots is handed over through HBM: the slot that
 // runs its head does so FIRST and raises flags[chain]; the next slot runs the tail LAST.
-__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int ring_me, int ring_next) {
+__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix) {
   const int lane = tix & 31, ww = tix >> 5, g = lane >> 2, t4 = lane & 3;
   const u32 gchain = p.chain_id_base + chain;
   // shared memory of this chain: exchange buffer(s), canonical weight and threshold rows, reduction and control words
@@ -665,7 +622,14 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
         td -= (u32)((int)p.tha[q] - (int)p.thb[q]) << (8 * j);
       }
     }
-    r.TA[w] = ta; r.TB[w] = ta + td;
+    if (CFOLD) {
+      r.CI[CFOLD ? w : 0][0] = ta & 0xFFFFu; r.CI[CFOLD ? w : 0][1] = ta & 0xFFFFu;
+      r.CI[CFOLD ? w : 0][2] = ta >> 16; r.CI[CFOLD ? w : 0][3] = ta >> 16;
+      asm volatile("" : "+r"(r.CI[CFOLD ? w : 0][0]), "+r"(r.CI[CFOLD ? w : 0][1]), "+r"(r.CI[CFOLD ? w : 0][2]), "+r"(r.CI[CFOLD ? w : 0][3]));
+      r.TB[w] = td;
+    } else {
+      r.TA[CFOLD ? 0 : w] = ta; r.TB[w] = ta + td;
+    }
   }
   if (MOVM) {
 #pragma unroll
@@ -698,7 +662,7 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     if (q1.is_w) xor_reg(r.A, q1.wsel, q1.wx);
     else if (q1.mine) shift_threshold(p, r, q1.loc, q1.oldv, q1.newv);
     // a3 / a4
-    const u32 fcand = simulate(p, r, sbuf, red, (int)(it & 1), lane, ww, ring_me, ring_next);
+    const u32 fcand = simulate(p, r, sbuf, red, (int)(it & 1), lane, ww);
     // a5
     u64 gs = p.g0 + (u64)it;
     if (REDERIVE) asm volatile("" : "+l"(gs));           // opaque: derive the proposal again instead of keeping it live

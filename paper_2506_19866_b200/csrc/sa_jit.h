@@ -23,10 +23,9 @@ struct StaticTuning {
   int dense_blocks = 0;   // dense kernel: resident chains (CTAs) per SM the register allocation aims at; 0 = 16 (128
                           // registers) with the sparse A operand, 12 (168 registers) with the dense one
   int dense_phases = 1;   // dense kernel: phases of a time step (accumulator tiles live at a time = row tiles / phases)
-  int dense_cpb = 1;      // dense kernel: one-warp chains per CTA (1, 4, 8 or 12); > 1 turns the tensor-pipe token ring on
+  int dense_cpb = 0;      // dense kernel: one-warp chains per CTA (1 .. 16, independent of one another); 0 = chosen from
+                          // the chain count: a CTA of 4k warps puts k chains on every SM sub-partition
   int dense_swizzle = 1;  // dense kernel: swizzled exchange buffer when it applies
-  int dense_lock = 0;     // dense kernel: tensor-pipe turn word (one CTA of dense_cpb one-warp chains per SM; TSD_LOCK in the kernel)
-  int dense_lock_rel = 3; // ... freed when the accumulator of this result word is complete
   int dense_movm = 0;     // dense kernel: exchange the states through registers (movmatrix) when one warp runs a chain;
                           // measured slower than the shared-memory exchange (143 against 148 M on Mtb-shaped), kept as an option
   int dense_sparse = 1;   // dense kernel: use the 2:4-sparse A operand (mma.sp) when the network allows it
@@ -43,7 +42,6 @@ bool static_kernel_compile(const std::vector<std::string>& defines, std::string*
 
 struct StaticKernel {
   int chains_per_cta = 1;
-  bool free_slots = true;     // dense kernel: the chains of a CTA run independently (no token ring), so balanced slots apply
   int blocks_per_sm = 0;      // resident CTAs per SM at this kernel's registers and shared memory (occupancy query)
   void* module = nullptr;     // CUmodule
   void* function = nullptr;   // CUfunction

@@ -296,7 +296,7 @@ def test_balanced_slots_hand_chains_over(B, problems_cache):
         B.sa_run(hd.h, 17)
         B.sa_run(hd.h, steps - 17)
         info = B.sa_get_info(hd.h)
-        assert info["variant"] == 5 and info["grid"] < R, info
+        assert info["variant"] == 5 and info["grid"] * info["chains_per_cta"] < R, info
         check_chains(B, hd, orc, chains, steps, B.sa_get_trace(hd.h, len(chains), steps))
         balanced = B.sa_get_fitness(hd.h, R)
     os.environ["TSA_DENSE_NO_BALANCE"] = "1"
@@ -304,7 +304,8 @@ def test_balanced_slots_hand_chains_over(B, problems_cache):
         with Handle(B, prob, sched) as hd:
             B.sa_select_kernel(hd.h, B.SA_KERNEL_DENSE)
             B.sa_run(hd.h, steps)
-            assert B.sa_get_info(hd.h)["grid"] == R
+            info = B.sa_get_info(hd.h)
+            assert info["grid"] == -(-R // info["chains_per_cta"]), info       # one chain per slot, no hand-over
             plain = B.sa_get_fitness(hd.h, R)
     finally:
         del os.environ["TSA_DENSE_NO_BALANCE"]
