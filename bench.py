@@ -303,7 +303,7 @@ def run_ours(args) -> dict:
              "peak_source": f"{sms} SMs x 4 schedulers x {sm_hz/1e6:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §7)",
              "kernel": kn, "kernel_ms": kernel_s * 1e3,
              # HBM traffic of the launch is the stage + write-back of the chains (2P + 8 bytes per chain each way,
-             # ~6 MB per launch in profiles/r1_v6_run_dense_sparse_unrolled.md); it is not re-measured in this run
+             # ~6 MB per launch in profiles/r2c_mtb_dense.md); it is not re-measured in this run
              "traffic": None,
              "alg_ops_per_chain_step": prob.alg_ops_per_step,
              "useful_frac": prob.alg_ops_per_step * rate / (issue_peak * 32)}
@@ -326,6 +326,15 @@ def run_ours(args) -> dict:
             r["tensor_pipe"] = {"imma_per_chain_step": per_step, "sparse_2of4": bool(di["sparse"]),
                                 "achieved_imma_per_s": per_step * rate, "peak_imma_per_s": peak,
                                 "peak_source": "sa_imma_peak, measured in this run", "frac": per_step * rate / peak}
+            # On this tensor path an IMMA holds its sub-partition's issue port for its whole slot: the rate above is
+            # one IMMA per 9 clocks per scheduler and nothing else issues meanwhile (measured: profiles/r2c_microbench.md,
+            # DESIGN.md §7).  Scheduler clocks accounted for = IMMA slots + one clock per other warp-instruction.
+            if r.get("warp_inst_per_chain_step"):
+                imma_clk = issue_peak / peak
+                clocks = per_step * imma_clk + (r["warp_inst_per_chain_step"] - per_step)
+                r["exclusive_issue"] = {"clocks_per_imma": imma_clk, "scheduler_clocks_per_chain_step": clocks,
+                                        "frac": clocks * rate / issue_peak,
+                                        "note": "fraction of scheduler clocks that hold an IMMA slot or issue another instruction"}
         return r
 
     name = args.workload
