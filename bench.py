@@ -313,6 +313,11 @@ def run_ours(args) -> dict:
             r["achieved"] = cnt["warp_inst_per_chain_step"] * rate / 1e12
             r["frac"] = cnt["warp_inst_per_chain_step"] * rate / issue_peak
             r["inst_per_node_update"] = cnt["warp_inst_per_chain_step"] / prob.node_updates_per_step
+            if cnt.get("smem_wavefronts_per_chain_step"):
+                # the gather kernels' ceiling is the shared-memory data pipe, one 128-byte wavefront per clock per SM
+                r["shared_pipe"] = {"wavefronts_per_chain_step": cnt["smem_wavefronts_per_chain_step"],
+                                    "source": cnt.get("smem_source"), "peak": "1 wavefront per clock per SM",
+                                    "frac": cnt["smem_wavefronts_per_chain_step"] * rate / (sms * sm_hz)}
         else:
             r["achieved"] = None
             r["frac"] = None
@@ -403,6 +408,8 @@ def run_ours(args) -> dict:
                 rf = roofline(wn, m["prob"], r, s, m, sms, sm_hz, imma)
                 extra[key] = {"value": v, "unit": UNIT, "node_updates_per_sec": v * m["prob"].node_updates_per_step,
                               "roofline_frac": rf["frac"], "useful_frac": rf["useful_frac"], "kernel": rf["kernel"],
+                              **({"exclusive_issue_frac": rf["exclusive_issue"]["frac"]} if "exclusive_issue" in rf else {}),
+                              **({"shared_pipe_frac": rf["shared_pipe"]["frac"]} if "shared_pipe" in rf else {}),
                               "ms_per_step": m["total_ms"] / 2, "repeats_identical": m["repeats_identical"], **m["info"]}
             if name == "mtb":
                 # the paper's level structure (Table 1) with the synchronisation on the device
