@@ -251,6 +251,11 @@ FAMILY_CASES = [
     ("hpg", "DENSE", {"TSA_DENSE_CPB": "4"}),
     ("mtb", "DENSE", {"TSA_DENSE_SP": "0"}), ("mtb", "DENSE", {"TSA_DENSE_SP": "0", "TSA_DENSE_W": "2"}),
     ("mtb", "DENSE", {"TSA_DENSE_SP": "0", "TSA_DENSE_CPB": "8"}),
+    # round 2: register exchange through movmatrix, thresholds folded into the C operand, chains per CTA
+    ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1"}), ("hpg", "DENSE", {"TSA_DENSE_MOVM": "1"}),
+    ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1", "TSA_DENSE_SP": "0"}), ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1", "TSA_DENSE_CPB": "16"}),
+    ("mtb", "DENSE", {"TSA_DENSE_CFOLD": "1"}), ("hpg", "DENSE", {"TSA_DENSE_CFOLD": "0"}), ("hpg", "DENSE", {"TSA_DENSE_CFOLD": "1", "TSA_DENSE_MOVM": "1"}),
+    ("mtb", "DENSE", {"TSA_DENSE_CPB": "1"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "7"}),
 ]
 
 
