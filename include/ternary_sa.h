@@ -179,7 +179,7 @@ int sa_get_dense_info(sa_handle *h, int64_t info[8]);
  * a result): TSA_TEAM_WARPS, TSA_TEAM_MIN, TSA_CPB, TSA_NO_SPLIT, TSA_NO_BANKOPT,
  * TSA_NO_TIERS, TSA_MAX_SLOTS (generic / static launch shape and host schedule); TSA_JIT_REGS,
  * TSA_JIT_BATCH, TSA_JIT_TUNROLL (static kernel); TSA_DENSE_BLOCKS, TSA_DENSE_PH, TSA_DENSE_CPB,
- * TSA_DENSE_SWZ, TSA_DENSE_SP, TSA_DENSE_MOVM, TSA_DENSE_W, TSA_DENSE_REDERIVE, TSA_DENSE_TUNROLL, TSA_DENSE_CFOLD,
+ * TSA_DENSE_SWZ, TSA_DENSE_SP, TSA_DENSE_MOVM, TSA_DENSE_W, TSA_DENSE_REDERIVE, TSA_DENSE_TUNROLL, TSA_DENSE_CFOLD, TSA_DENSE_SPEC,
  * TSA_DENSE_NO_BALANCE (dense kernel); TSA_PAPER_LPC, TSA_PAPER_WPB, TSA_PAPER_BLOCKS (paper model);
  * TSA_BOUNDS_CHECK=1 compiles the run-time kernels with shared-memory bounds checks that trap (debug);
  * TSA_JIT_DUMP=<dir> keeps every run-time compiled cubin and its option list there (for cuobjdump). */

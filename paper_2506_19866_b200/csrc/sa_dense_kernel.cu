@@ -60,6 +60,9 @@
 #ifndef TSD_CFOLD
 #define TSD_CFOLD 0
 #endif
+#ifndef TSD_SPEC
+#define TSD_SPEC 1
+#endif
 #ifndef TSD_FIXW_MASK
 #define TSD_FIXW_MASK 0
 #endif
@@ -108,7 +111,17 @@ __host__ __device__ constexpr int popc_below(u32 m, int w) { int n = 0; for (int
 constexpr int NFW = popc_below(kFixW, 32) > 0 ? popc_below(kFixW, 32) : 1;
 constexpr int STATE_BYTES = MOVM ? 0 : SWZ ? 1024 : 8 * CS;   // one exchange buffer: 8 condition rows
 constexpr int NBUF = TW > 1 ? 2 : 1;            // teams alternate between two exchange buffers: one barrier per time step
-constexpr int CHAIN_SMEM = (NBUF * STATE_BYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 8) * 4 + 15) / 16 * 16;   // bytes per chain
+// Speculative look-ahead (TSD_SPEC = D > 1, one-warp chains): D warps hold the same chain and evaluate the proposals
+// of the SA steps g .. g+D-1 against the same current vector at the same time; the steps up to and including the
+// first accepted one are what the serial chain would have done (a rejected step leaves the vector unchanged, and
+// proposal, level and random numbers of a step depend on (seed, chain, g) alone), so they are consumed and the rest
+// is thrown away: bit-exact, 1 + r + r^2 + ... steps per pass at rejection rate r.  It pays where the chains
+// are too few to fill the GPU (HPG-shaped: 1024 chains, 7 warps per SM); see run_spec below.
+constexpr int SPEC = TSD_SPEC;
+static_assert(SPEC >= 1 && SPEC <= 4 && (SPEC == 1 || TSD_W == 1), "look-ahead depth 1 .. 4, one-warp chains");
+constexpr int RES_WORDS = SPEC > 1 ? 2 * SPEC : 0;      // per warp of a chain: its step's flags and candidate fitness
+constexpr int XBYTES = NBUF * STATE_BYTES;              // exchange buffer(s) of one warp team
+constexpr int CHAIN_SMEM = (SPEC * XBYTES + TSD_EPADA + TSD_NPADA + (2 * TW + 8 + RES_WORDS) * 4 + 15) / 16 * 16;   // bytes per chain
 // The host numbers the observed nodes first, so only the result words w < OBSW hold scored entries; the observation
 // words of a lane and time are stored w-major ([w][c]) and fetched with vector loads.
 constexpr int OBSW = TSD_OBSW;
@@ -136,6 +149,7 @@ static_assert(!MOVM || TSD_W == 1, "the register exchange is for one warp per ch
 static_assert(WPW >= 1 && WPW * TW == NW, "team width must divide the words per condition");
 static_assert(WPP >= 1 && WPP * PH == WPW, "phases must divide the words of a warp");
 static_assert(CPB == 1 || (TW == 1 && CPB <= 16), "several chains per CTA: one-warp chains");
+static_assert(TSD_SPEC == 1 || (TSD_CPB <= 15 && TSD_CPB * TSD_SPEC <= 32), "look-ahead: one named barrier per chain, at most 32 warps per CTA");
 // Philox4x32-10 (Salmon et al., SC'11)
 __device__ __forceinline__ void philox4x32_10(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1, u32 (&out)[4]) {
 #pragma unroll
@@ -190,6 +204,12 @@ __device__ __forceinline__ void imma_sp_c(int (&c)[4], const u32* a, u32 b0, u32
 
 __device__ __forceinline__ void team_sync() {
   if (TW == 1) __syncwarp(); else __syncthreads();
+}
+
+// the SPEC warps that hold chain slot wc of the CTA (named barrier 1 + wc); one team otherwise
+__device__ __forceinline__ void group_sync(int wc) {
+  if (SPEC == 1) team_sync();
+  else asm volatile("bar.sync %0, %1;" ::"r"(1 + wc), "n"(32 * TSD_SPEC) : "memory");
 }
 
 // Debug build (-DTSA_BOUNDS=1, set by TSA_BOUNDS_CHECK=1 under TSA_TUNING=1): every shared-memory access made
@@ -524,7 +544,8 @@ __device__ __forceinline__ void shift_threshold(const Params& p, Regs& r, u32 lo
     }
 }
 
-__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix);
+__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int wc, int sd);
+
 
 // add the piece's counts of level ctl[6] to the handle's table and clear them (one thread per chain)
 __device__ __noinline__ void flush_stats(const Params& p, volatile u32* ctl) {
@@ -535,9 +556,10 @@ __device__ __noinline__ void flush_stats(const Params& p, volatile u32* ctl) {
   ctl[2] = 0u; ctl[3] = 0u; ctl[4] = 0u; ctl[5] = 0u;
 }
 
-extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_dense(const __grid_constant__ Params p) {
+extern "C" __global__ void __launch_bounds__(TEAM * CPB * SPEC, TSD_MINBLOCKS) tsa_run_dense(const __grid_constant__ Params p) {
   extern __shared__ __align__(16) u32 smem_all[];
-  const int tix = threadIdx.x % TEAM, wc = threadIdx.x / TEAM;       // thread within the chain's team, chain slot within the CTA
+  const int tix = threadIdx.x % TEAM;                                 // thread within the chain's team
+  const int wc = threadIdx.x / (TEAM * SPEC), sd = threadIdx.x / TEAM % SPEC;   // chain slot within the CTA, look-ahead position
   const u32 chain = blockIdx.x * CPB + wc;
   if (p.slot_steps == 0 && chain >= (u32)p.R) return;
   u32* const smem = smem_all + (size_t)wc * (CHAIN_SMEM / 4);
@@ -559,7 +581,99 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
     const bool head_first = cb > ca && hi < (cb + 1) * S;
     const i64 c = n == count - 1 ? ca : head_first ? (n == 0 ? cb : ca + n) : ca + 1 + n;
     const i64 b0 = c * S;
-    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix);
+    run_piece(p, (u32)c, (lo > b0 ? lo : b0) - b0, (hi < b0 + S ? hi : b0 + S) - b0, smem, tix, wc, sd);
+  }
+}
+
+
+// temperature level of SA step gs (reading 20)
+__device__ __forceinline__ u64 level_of(const Params& p, u64 gs) {
+  u64 level = ((gs | (u64)p.steps_per_level) >> 32) == 0 ? (u64)((u32)gs / (u32)p.steps_per_level) : gs / (u64)p.steps_per_level;
+  if (level > (u64)(p.n_levels - 1)) level = (u64)(p.n_levels - 1);
+  return level;
+}
+
+// The SA steps [s0, s1) of one chain with look-ahead (SPEC warps per chain, this one at position sd).  One pass:
+// warp sd proposes and scores step it + sd against the current vector and posts (live, accepted, fitness); after the
+// first barrier every warp knows the first accepted position a and the number of steps consumed (a + 1, or all live
+// ones); warps other than a take their own change back and, if there is an a, apply step it + a's change to their
+// registers (derived again from the canonical rows, which are still the old ones); after the second barrier warp a
+// commits to the canonical rows and control words; the consumed warps write their trace records, warp 0 keeps the
+// level statistics; the third barrier ends the pass.
+__device__ __forceinline__ void run_spec(const Params& p, Regs& r, u32 chain, u32 gchain, i64 s0, i64 s1, u32 sbuf, i8* cw, i8* cth,
+                                         volatile u32* red, volatile u32* ctl, int lane, int wc, int sd) {
+  const int g = lane >> 2, t4 = lane & 3;
+  volatile u32* const res = ctl + 8;                     // [2 * position] bit 1 live, bit 0 accepted; [2 * position + 1] candidate fitness
+  const int trow = p.trace_row ? __ldg(p.trace_row + chain) : -1;
+#pragma unroll 1
+  for (i64 it = s0; it < s1;) {
+    const i64 my = it + sd;
+    const bool live = my < s1;                           // warp-uniform
+    const u32 fcur = ctl[0], fbest = ctl[1];
+    Proposal q;
+    u32 fcand = 0u;
+    bool acc = false;
+    i64 d = 0;
+    if (live) {
+      q = propose(p, p.g0 + (u64)my, gchain, lane, 0, g, cw, cth);
+      if (q.is_w) xor_reg(r.A, q.wsel, q.wx);
+      else if (q.mine) shift_threshold(p, r, q.loc, q.oldv, q.newv);
+      fcand = simulate(p, r, sbuf, red, 0, lane, 0);
+      d = (i64)fcand - (i64)fcur;
+      acc = d <= 0;
+      if (!acc && d <= (i64)p.dmax) acc = q.x2 < __ldg(p.accept + level_of(p, p.g0 + (u64)my) * (u64)p.dmax + (u64)(d - 1));
+    }
+    if (lane == 0) { res[2 * sd] = live ? (acc ? 3u : 2u) : 0u; res[2 * sd + 1] = fcand; }
+    group_sync(wc);
+    int a = -1, consumed = 0;
+#pragma unroll
+    for (int j = 0; j < SPEC; ++j) {
+      const u32 f = res[2 * j];
+      if (a < 0 && consumed == j && (f & 2u)) { consumed = j + 1; if (f & 1u) a = j; }
+    }
+    if (live && sd != a) {                               // not the accepted step: the change is taken back
+      if (q.is_w) xor_reg(r.A, q.wsel, q.wx);
+      else if (q.mine) shift_threshold(p, r, q.loc, q.newv, q.oldv);
+    }
+    if (a >= 0 && sd != a) {                             // the accepted step's change, from the still unchanged canonical rows
+      const Proposal qa = propose(p, p.g0 + (u64)(it + a), gchain, lane, 0, g, cw, cth);
+      if (qa.is_w) xor_reg(r.A, qa.wsel, qa.wx);
+      else if (qa.mine) shift_threshold(p, r, qa.loc, qa.oldv, qa.newv);
+    }
+    if (p.level_stats && sd == 0 && lane == 0) {
+      for (int j = 0; j < consumed; ++j) {
+        const u32 lv = (u32)level_of(p, p.g0 + (u64)(it + j)), fj = res[2 * j + 1];
+        if (lv != ctl[6]) { flush_stats(p, ctl); ctl[6] = lv; }
+        ctl[2] += 1u;
+        if (j == a) { ctl[3] += 1u; ctl[4] += fj > fcur ? 1u : 0u; ctl[5] += fj < fbest ? 1u : 0u; }
+      }
+    }
+    group_sync(wc);                                      // everyone has read the canonical rows and the control words
+    const bool new_best = sd == a && fcand < fbest;
+    if (sd == a) {
+      if (lane == 0) { ctl[0] = fcand; if (new_best) ctl[1] = fcand; }
+      if (q.mine) {
+        if (q.is_w) cw[q.slot] = (i8)q.newv;
+        else if (t4 == 0) cth[q.slot] = (i8)q.newv;
+      }
+      if (new_best) {
+        __syncwarp();
+        u32* const best_w = (u32*)(p.best_w + (size_t)chain * TSD_EPADA);
+        u32* const best_th = (u32*)(p.best_th + (size_t)chain * TSD_NPADA);
+        for (int i = lane; i < TSD_EPADA / 4; i += 32) best_w[i] = ((const u32*)cw)[i];
+        for (int i = lane; i < TSD_NPADA / 4; i += 32) best_th[i] = ((const u32*)cth)[i];
+      }
+    }
+    if (trow >= 0 && sd < consumed && q.mine && (q.is_w || t4 == 0)) {
+      const u64 gs = p.g0 + (u64)my, idx = gs - p.trace_g0;
+      const u32 code = q.is_w ? (u32)(q.newv + 1) : (u32)q.newv;
+      if (gs >= p.trace_g0 && idx < (u64)p.trace_max)
+        p.trace_rec[(size_t)trow * (size_t)p.trace_max + idx] =
+            (u64)fcand | ((u64)q.pidx << 32) | ((u64)code << 56) | ((u64)(sd == a ? 1 : 0) << 60) | ((u64)(new_best ? 1 : 0) << 61) |
+            ((u64)(q.moved ? 0 : 1) << 62);
+    }
+    group_sync(wc);                                      // the commit is visible
+    it += consumed;
   }
 }
 
@@ -568,14 +682,16 @@ extern "C" __global__ void __launch_bounds__(TEAM * CPB, TSD_MINBLOCKS) tsa_run_
 // are more chains than resident slots the host splits the (chain, step) line evenly over the slots
 // (slot_steps > 0), and a chain that straddles two slots is handed over through HBM: the slot that
 // runs its head does so FIRST and raises flags[chain]; the next slot runs the tail LAST.
-__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix) {
+__device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i64 s1, u32* smem, int tix, int wc, int sd) {
   const int lane = tix & 31, ww = tix >> 5, g = lane >> 2, t4 = lane & 3;
   const u32 gchain = p.chain_id_base + chain;
-  // shared memory of this chain: exchange buffer(s), canonical weight and threshold rows, reduction and control words
-  i8* const cw = (i8*)smem + NBUF * STATE_BYTES;
+  // shared memory of this chain: exchange buffer(s) (one set per look-ahead warp), canonical weight and threshold rows,
+  // reduction and control words, look-ahead results
+  i8* const cw = (i8*)smem + SPEC * XBYTES;
   i8* const cth = cw + TSD_EPADA;
   volatile u32* const red = (volatile u32*)(cth + TSD_NPADA);
-  const u32 sbuf = (u32)__cvta_generic_to_shared(smem);
+  u32* const xbuf = smem + (SPEC > 1 ? sd * (XBYTES / 4) : 0);
+  const u32 sbuf = (u32)__cvta_generic_to_shared(xbuf);
   // (row addresses are formed where they are used, never held across the time loop)
 
   if (s0 > 0) {                              // the head of this chain is another slot's first piece
@@ -592,10 +708,12 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     team_sync();
   }
   // a0: stage the chain
-  for (int x = tix; x < NBUF * STATE_BYTES / 4; x += TEAM) smem[x] = 0u;
-  for (int x = tix; x < TSD_EPADA / 4; x += TEAM) ((u32*)cw)[x] = __ldcg((const u32*)(p.cur_w + (size_t)chain * TSD_EPADA) + x);
-  for (int x = tix; x < TSD_NPADA / 4; x += TEAM) ((u32*)cth)[x] = __ldcg((const u32*)(p.cur_th + (size_t)chain * TSD_NPADA) + x);
-  team_sync();
+  for (int x = tix; x < XBYTES / 4; x += TEAM) xbuf[x] = 0u;
+  if (SPEC == 1 || sd == 0) {
+    for (int x = tix; x < TSD_EPADA / 4; x += TEAM) ((u32*)cw)[x] = __ldcg((const u32*)(p.cur_w + (size_t)chain * TSD_EPADA) + x);
+    for (int x = tix; x < TSD_NPADA / 4; x += TEAM) ((u32*)cth)[x] = __ldcg((const u32*)(p.cur_th + (size_t)chain * TSD_NPADA) + x);
+  }
+  group_sync(wc);
   Regs r;
 #pragma unroll
   for (int i = 0; i < NA; ++i) {
@@ -651,11 +769,12 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
   // registers across the time loop: the register budget there decides warps per SM.
   volatile u32* const ctl = red + 2 * TW;               // [0] d_cur, [1] d_best, [2..5] steps / accepted / accepted worse / new best
                                                         // of the level [6] this piece is running, thread 0 only
-  if (tix == 0) { ctl[0] = __ldcg(p.fit_cur + chain); ctl[1] = __ldcg(p.fit_best + chain); ctl[2] = 0u; ctl[6] = 0xFFFFFFFFu; }
-  team_sync();
+  if (tix == 0 && (SPEC == 1 || sd == 0)) { ctl[0] = __ldcg(p.fit_cur + chain); ctl[1] = __ldcg(p.fit_best + chain); ctl[2] = 0u; ctl[6] = 0xFFFFFFFFu; }
+  group_sync(wc);
 
+  if (SPEC > 1) run_spec(p, r, chain, gchain, s0, s1, sbuf, cw, cth, red, ctl, lane, wc, sd);
 #pragma unroll 1
-  for (i64 it = s0; it < s1; ++it) {
+  for (i64 it = s0; SPEC == 1 && it < s1; ++it) {
     // a1 / a2: propose; the threads that hold the parameter apply it in their registers.  Only they
     // read or write its byte in the canonical row, so the row needs no barrier of its own.
     const Proposal q1 = propose(p, p.g0 + (u64)it, gchain, lane, ww, g, cw, cth);
@@ -710,16 +829,18 @@ __device__ __forceinline__ void run_piece(const Params& p, u32 chain, i64 s0, i6
     }
   }
   // a7
-  team_sync();
-  for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)(p.cur_w + (size_t)chain * TSD_EPADA))[i] = ((const u32*)cw)[i];
-  for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)(p.cur_th + (size_t)chain * TSD_NPADA))[i] = ((const u32*)cth)[i];
-  if (tix == 0) { p.fit_cur[chain] = ctl[0]; p.fit_best[chain] = ctl[1]; if (p.level_stats) flush_stats(p, ctl); }
-  if (s1 < p.steps) {                        // hand the chain over
-    __threadfence();
-    team_sync();
-    if (tix == 0) { __threadfence(); atomicExch(p.flags + chain, 1u); }
+  group_sync(wc);
+  if (SPEC == 1 || sd == 0) {
+    for (int i = tix; i < TSD_EPADA / 4; i += TEAM) ((u32*)(p.cur_w + (size_t)chain * TSD_EPADA))[i] = ((const u32*)cw)[i];
+    for (int i = tix; i < TSD_NPADA / 4; i += TEAM) ((u32*)(p.cur_th + (size_t)chain * TSD_NPADA))[i] = ((const u32*)cth)[i];
+    if (tix == 0) { p.fit_cur[chain] = ctl[0]; p.fit_best[chain] = ctl[1]; if (p.level_stats) flush_stats(p, ctl); }
+    if (s1 < p.steps) {                        // hand the chain over
+      __threadfence();
+      team_sync();
+      if (tix == 0) { __threadfence(); atomicExch(p.flags + chain, 1u); }
+    }
   }
-  team_sync();                               // the shared memory is free for the next piece
+  group_sync(wc);                            // the shared memory is free for the next piece
 }
 
 }  // namespace tsa_dense

@@ -33,8 +33,9 @@ struct DensePlan {
   std::vector<uint32_t> fix;         // [W][n_fix_rounds][32]; register exchange: [n_fix_rounds][2][2][32] keep / value masks
   std::vector<uint32_t> wloc;        // [E]
   std::vector<uint32_t> thloc;       // [N]
-  size_t smem_bytes(const Plan& pl) const {   // per chain, as CHAIN_SMEM in the kernel
-    return ((size_t)(W > 1 ? 2 : 1) * (movm ? 0 : swizzle ? 1024 : 8 * CS) + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 8) * 4 + 15) / 16 * 16;
+  size_t smem_bytes(const Plan& pl, int spec = 1) const {   // per chain, as CHAIN_SMEM in the kernel (spec = look-ahead warps)
+    const size_t xbytes = (size_t)(W > 1 ? 2 : 1) * (movm ? 0 : swizzle ? 1024 : 8 * CS);
+    return ((size_t)spec * xbytes + (size_t)pl.EpadA + (size_t)pl.NpadA + (size_t)(2 * W + 8 + (spec > 1 ? 2 * spec : 0)) * 4 + 15) / 16 * 16;
   }
 };
 

@@ -26,6 +26,7 @@ struct StaticTuning {
   int dense_cpb = 0;      // dense kernel: one-warp chains per CTA (1 .. 16, independent of one another); 0 = chosen from
                           // the chain count: a CTA of 4k warps puts k chains on every SM sub-partition
   int dense_swizzle = 1;  // dense kernel: swizzled exchange buffer when it applies
+  int dense_spec = 1;     // dense kernel: look-ahead depth (warps per one-warp chain that score consecutive SA steps at once)
   int dense_movm = 0;     // dense kernel: exchange the states through registers (movmatrix) when one warp runs a chain;
                           // measured slower than the shared-memory exchange (143 against 148 M on Mtb-shaped), kept as an option
   int dense_sparse = 1;   // dense kernel: use the 2:4-sparse A operand (mma.sp) when the network allows it
@@ -62,6 +63,8 @@ std::vector<std::string> dense_kernel_defines(const Plan& plan, const DensePlan&
 bool dense_kernel_compile(const std::vector<std::string>& defines, std::string* cubin, std::string* log);
 // chains per CTA the kernel will be built for (1 unless the plan has one-warp chains)
 int dense_chains_per_cta(const DensePlan& dp, const StaticTuning& tune);
+// look-ahead depth the kernel will be built with (1 unless the plan has one-warp chains)
+int dense_look_ahead(const DensePlan& dp, const StaticTuning& tune);
 const StaticKernel* dense_kernel_get(const Plan& plan, const DensePlan& dp, const StaticTuning& tune, std::string* why);
 // cooperative = true: cuLaunchCooperativeKernel (every CTA of the grid resident at once, or the launch fails)
 int dense_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_dense::Params& params, std::string* why,

@@ -54,7 +54,8 @@ def test_every_chain_starts_from_a_valid_vector(B, problems_cache, name, R):
 
 CASES = [("hpg", "STATIC", {}), ("mtb", "STATIC", {}), ("hpg", "GENERIC", {}), ("hpg", "GENERIC", {"TSA_KERNEL": "cta"}), ("hpg", "DENSE", {}), ("hpg", "AUTO", {}),
          ("mtb", "GENERIC", {}), ("mtb", "DENSE", {}), ("mtb", "DENSE", {"TSA_DENSE_SP": "0"}), ("mtb", "DENSE", {"TSA_DENSE_W": "2"}),
-         ("mtb", "AUTO", {}), ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "16"})]
+         ("mtb", "AUTO", {}), ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "16"}),
+         ("hpg", "DENSE", {"TSA_DENSE_SPEC": "3"}), ("mtb", "DENSE", {"TSA_DENSE_SPEC": "2"})]
 
 
 @pytest.mark.parametrize("name,family,env", CASES, ids=[f"{n}-{f}-{'-'.join(e.values()) or 'default'}" for n, f, e in CASES])

@@ -256,6 +256,10 @@ FAMILY_CASES = [
     ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1", "TSA_DENSE_SP": "0"}), ("mtb", "DENSE", {"TSA_DENSE_MOVM": "1", "TSA_DENSE_CPB": "16"}),
     ("mtb", "DENSE", {"TSA_DENSE_CFOLD": "1"}), ("hpg", "DENSE", {"TSA_DENSE_CFOLD": "0"}), ("hpg", "DENSE", {"TSA_DENSE_CFOLD": "1", "TSA_DENSE_MOVM": "1"}),
     ("mtb", "DENSE", {"TSA_DENSE_CPB": "1"}), ("mtb", "DENSE", {"TSA_DENSE_CPB": "7"}),
+    # speculative look-ahead: 2 .. 4 warps per chain score consecutive SA steps at once
+    ("hpg", "DENSE", {"TSA_DENSE_SPEC": "2"}), ("hpg", "DENSE", {"TSA_DENSE_SPEC": "3", "TSA_DENSE_CPB": "7"}),
+    ("hpg", "DENSE", {"TSA_DENSE_SPEC": "4", "TSA_DENSE_CPB": "4"}), ("mtb", "DENSE", {"TSA_DENSE_SPEC": "2", "TSA_DENSE_CPB": "8"}),
+    ("mtb", "DENSE", {"TSA_DENSE_SPEC": "3", "TSA_DENSE_SP": "0"}), ("hpg", "DENSE", {"TSA_DENSE_SPEC": "2", "TSA_DENSE_MOVM": "1"}),
 ]
 
 
