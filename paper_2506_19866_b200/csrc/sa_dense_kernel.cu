@@ -63,6 +63,7 @@
 #ifndef TSD_SPEC
 #define TSD_SPEC 1
 #endif
+
 #ifndef TSD_FIXW_MASK
 #define TSD_FIXW_MASK 0
 #endif
@@ -279,9 +280,13 @@ struct Phases {
   template <int KK>
   static __device__ __forceinline__ void one(const Regs& r, const u32 (&bh)[2 * KS], const u32 (&bl)[2 * KS], int n_tiles,
                                              int (&acc)[4], int w, int step) {
-    const int tile = 2 * (P * WPP + w) + step / KK, s = step % KK;
+    // (with an even number of row tiles the odd tile of a pair goes first: it takes the exchanged bytes as they are,
+    // and the shift that makes the even tile's operand is off the chain's critical path)
+    constexpr bool kOddFirst = MT % 2 == 0 && TSD_W == 1;
+    const int odd = kOddFirst ? 1 - step / KK : step / KK;
+    const int tile = 2 * (P * WPP + w) + odd, s = step % KK;
     if (!(TW * MTW <= MT || tile < n_tiles)) return;
-    const u32* bb = step / KK ? bh : bl;
+    const u32* bb = odd ? bh : bl;
     if (CFOLD && step == 0) {
       if (SP) imma_sp_c(acc, &r.A[(tile * KSP + s) * 4], bb[4 * s], bb[4 * s + 1], bb[4 * s + 2], bb[4 * s + 3], r.M[SP ? tile * KSP + s : 0], r.CI[CFOLD ? P * WPP + w : 0]);
       else imma_c(acc, &r.A[(tile * KS + s) * 4], bb[2 * s], bb[2 * s + 1], r.CI[CFOLD ? P * WPP + w : 0]);
