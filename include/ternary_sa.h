@@ -84,7 +84,9 @@ typedef struct {
  * accumulator range: 128 + s - th_lo[q] and 128 + s - th_hi[q] - 1 in [0,255] for all |s| <=
  * 2*max_in_degree (in-degree <= 62 with thresholds in [-3,3]); kernel limits: n_pairs in [2,16],
  * n_steps <= 127, n_obs <= 127, E < 2^24, state entries x words per entry x 4 <= 65535 bytes (about
- * 16 000 nodes at K <= 4, 4 000 at K <= 16).  On failure *out = NULL. */
+ * 16 000 nodes at K <= 4, 4 000 at K <= 16).  On failure *out = NULL.
+ * The host-side plans of a problem (tens of milliseconds) are kept, keyed by the problem's bytes, for the next
+ * sa_create on the same problem (the last eight problems; thread safe). */
 int sa_create(const sa_network *net, const sa_observations *obs, const sa_schedule *sched, sa_handle **out);
 
 /* Advance every chain by `steps` SA steps (Table 1 inner loop :130-149; SURVEY.md

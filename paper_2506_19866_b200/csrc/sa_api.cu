@@ -4,7 +4,9 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <map>
 #include <memory>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -249,6 +251,30 @@ tsa::PlanOptions plan_options(int64_t n_chains, int sm_count) {
   return o;
 }
 
+// Host plans (edge schedule, bank classes, 2:4 row search, fragment tables) are a pure function of the problem and
+// the options, and take tens of milliseconds: sa_create keeps the last few, keyed by the problem's bytes, so that a
+// second handle on the same problem (another chain range, another schedule, a restart) only pays for the device side.
+struct CachedPlans { tsa::Plan plan; tsa::DensePlan dplan; };
+std::mutex g_plans_mu;
+std::map<std::string, std::shared_ptr<const CachedPlans>> g_plans;
+
+bool plan_key(const sa_network* net, const sa_observations* obs, const tsa::PlanOptions& o, const tsa::StaticTuning& t, std::string* key) {
+  if (net->n_nodes <= 0 || net->n_edges <= 0 || net->n_pairs <= 0 || net->n_pairs > 16 || !net->edge_src || !net->edge_dst ||
+      !net->th_lo || !net->th_hi || obs->n_cond <= 0 || obs->n_steps <= 0 || obs->n_obs <= 0 || !obs->obs_times ||
+      !obs->init_state || !obs->clamp || !obs->obs)
+    return false;                                        // let build_plan say what is wrong
+  const size_t N = (size_t)net->n_nodes, E = (size_t)net->n_edges, K = (size_t)obs->n_cond, NO = (size_t)obs->n_obs;
+  if (N > 100000 || E > 10000000 || K > 1024 || NO > 100000) return false;
+  auto put = [&](const void* ptr, size_t n) { key->append((const char*)ptr, n); };
+  const int32_t head[] = {net->n_nodes, net->n_edges, net->n_pairs, obs->n_cond, obs->n_steps, obs->n_obs, (int32_t)o.split_rows,
+                          (int32_t)o.bank_opt, (int32_t)o.tiers, o.min_team_warps, o.max_lane_slots, t.dense_warps, t.dense_sparse,
+                          t.dense_swizzle, t.dense_movm};
+  put(head, sizeof(head));
+  put(net->edge_src, E * 4); put(net->edge_dst, E * 4); put(net->th_lo, (size_t)net->n_pairs); put(net->th_hi, (size_t)net->n_pairs);
+  put(obs->obs_times, NO * 4); put(obs->init_state, K * N); put(obs->clamp, K * N); put(obs->obs, K * NO * N);
+  return true;
+}
+
 }  // namespace
 
 extern "C" {
@@ -287,8 +313,33 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
   int dev = 0;
   cudaError_t dev_err = cudaGetDevice(&dev);
   if (dev_err == cudaSuccess) dev_err = cudaDeviceGetAttribute(&h->sm_count, cudaDevAttrMultiProcessorCount, dev);
-  int rc = tsa::build_plan(net, obs, true, plan_options(sched->n_chains, h->sm_count), &h->plan, &err);
-  if (rc != SA_OK) return set_err(rc, err);
+  int rc = SA_OK;
+  {
+    const tsa::PlanOptions popt = plan_options(sched->n_chains, h->sm_count);
+    const tsa::StaticTuning tune = tsa::StaticTuning::from_env();
+    std::string key;
+    const bool keyed = plan_key(net, obs, popt, tune, &key);
+    std::shared_ptr<const CachedPlans> hit;
+    if (keyed) {
+      std::lock_guard<std::mutex> lock(g_plans_mu);
+      auto it = g_plans.find(key);
+      if (it != g_plans.end()) hit = it->second;
+    }
+    if (hit) {
+      h->plan = hit->plan; h->dplan = hit->dplan;
+    } else {
+      rc = tsa::build_plan(net, obs, true, popt, &h->plan, &err);
+      if (rc != SA_OK) return set_err(rc, err);
+      tsa::build_dense_plan(net, obs, h->plan, tune.dense_warps, tune.dense_sparse != 0, tune.dense_swizzle != 0, tune.dense_movm != 0, &h->dplan);
+      if (keyed) {
+        auto entry = std::make_shared<CachedPlans>();
+        entry->plan = h->plan; entry->dplan = h->dplan;
+        std::lock_guard<std::mutex> lock(g_plans_mu);
+        if (g_plans.size() >= 8) g_plans.clear();
+        g_plans[key] = entry;
+      }
+    }
+  }
   if (sched->flags & ~(SA_LEVEL_STATS | SA_CONSTRAINED)) return set_err(SA_EINVAL, "unknown schedule flag");
   if (sched->flags & SA_CONSTRAINED) {
     std::vector<char> has_in(net->n_nodes, 0), has_out(net->n_nodes, 0);
@@ -307,8 +358,6 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
     if ((rc = h->pool.upload(h->plan.wloc, &h->d_wloc, st))) return rc;
     if ((rc = h->pool.upload(h->plan.thloc, &h->d_thloc, st))) return rc;
   }
-  tsa::build_dense_plan(net, obs, h->plan, tsa::StaticTuning::from_env().dense_warps, tsa::StaticTuning::from_env().dense_sparse != 0,
-                        tsa::StaticTuning::from_env().dense_swizzle != 0, tsa::StaticTuning::from_env().dense_movm != 0, &h->dplan);
   if (h->dplan.ok) {
     if ((rc = h->pool.upload(h->dplan.frag_slot, &h->d_frag_slot, st))) return rc;
     if ((rc = h->pool.upload(h->dplan.th_entry, &h->d_th_entry, st))) return rc;
