@@ -58,7 +58,24 @@ def embed_static_source() -> None:
                 f.write(text)
 
 
+MICRO = os.path.join(CSRC, "microbench")
+MICRO_OUT = os.path.join(HERE, "build")
+
+
+def build_microbench(force: bool = False) -> None:
+    """The stand-alone microbenchmarks behind the roofline (csrc/microbench/*.cu -> build/<name>, run by hand on a B200;
+    profiles/r2c_microbench.md has their output)."""
+    os.makedirs(MICRO_OUT, exist_ok=True)
+    for f in sorted(os.listdir(MICRO)):
+        if not f.endswith(".cu"):
+            continue
+        src, out = os.path.join(MICRO, f), os.path.join(MICRO_OUT, f[:-3])
+        if force or not os.path.exists(out) or os.path.getmtime(src) > os.path.getmtime(out):
+            subprocess.check_call([_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O2", "-o", out, src])
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
+    build_microbench(force)
     if not force and not stale():
         return LIB
     embed_static_source()
