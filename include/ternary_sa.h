@@ -178,7 +178,7 @@ int sa_get_dense_info(sa_handle *h, int64_t info[8]);
  * Environment.  Always read: TSA_KERNEL=generic|static|dense overrides sa_select_kernel (also cta|warp:
  * the generic family with one CTA / one warp per chain); TSA_NVRTC_LIB=<path> names the libnvrtc to load.
  * Read ONLY when TSA_TUNING=1 (measurements and the parity tests, which show that none of them changes
- * a result): TSA_TEAM_WARPS, TSA_TEAM_MIN, TSA_CPB, TSA_NO_SPLIT, TSA_NO_BANKOPT,
+ * a result): TSA_TEAM_WARPS, TSA_TEAM_MIN, TSA_CPB, TSA_NO_SPLIT, TSA_NO_BANKOPT, TSA_NO_STOREOPT,
  * TSA_NO_TIERS, TSA_MAX_SLOTS (generic / static launch shape and host schedule); TSA_JIT_REGS,
  * TSA_JIT_BATCH, TSA_JIT_TUNROLL (static kernel); TSA_DENSE_BLOCKS, TSA_DENSE_PH, TSA_DENSE_CPB,
  * TSA_DENSE_SWZ, TSA_DENSE_SP, TSA_DENSE_MOVM, TSA_DENSE_W, TSA_DENSE_REDERIVE, TSA_DENSE_TUNROLL, TSA_DENSE_CFOLD, TSA_DENSE_SPEC,

@@ -267,7 +267,7 @@ bool plan_key(const sa_network* net, const sa_observations* obs, const tsa::Plan
   if (N > 100000 || E > 10000000 || K > 1024 || NO > 100000) return false;
   auto put = [&](const void* ptr, size_t n) { key->append((const char*)ptr, n); };
   const int32_t head[] = {net->n_nodes, net->n_edges, net->n_pairs, obs->n_cond, obs->n_steps, obs->n_obs, (int32_t)o.split_rows,
-                          (int32_t)o.bank_opt, (int32_t)o.tiers, o.min_team_warps, o.max_lane_slots, t.dense_warps, t.dense_sparse,
+                          (int32_t)o.bank_opt, (int32_t)o.store_opt, (int32_t)o.tiers, o.min_team_warps, o.max_lane_slots, t.dense_warps, t.dense_sparse,
                           t.dense_swizzle, t.dense_movm};
   put(head, sizeof(head));
   put(net->edge_src, E * 4); put(net->edge_dst, E * 4); put(net->th_lo, (size_t)net->n_pairs); put(net->th_hi, (size_t)net->n_pairs);

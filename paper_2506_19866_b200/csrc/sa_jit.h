@@ -17,8 +17,10 @@
 namespace tsa {
 
 struct StaticTuning {
-  int max_regs = 128;     // register budget per thread -> __launch_bounds__ min blocks
-  int batch = 8;          // state gathers issued back to back before their IMADs
+  int max_regs = 0;       // static kernel: register budget per thread -> __launch_bounds__ min blocks; 0 = from the edge
+                          // slots a thread holds (measured on a B200: < 24 slots 128, 24 .. 43 slots 168 -- Mtb-shaped 70.9
+                          // -> 75.9 M chain-steps/s --, more 255 with 12 gathers in flight -- Large 3.50 -> 3.73 M)
+  int batch = 0;          // state gathers issued back to back before their IMADs; 0 = 8, or 12 at 255 registers
   int t_unroll = 1;       // unroll factor of the time loop
   int dense_blocks = 0;   // dense kernel: resident chains (CTAs) per SM the register allocation aims at; 0 = 16 (128
                           // registers) with the sparse A operand, 12 (168 registers) with the dense one

@@ -102,15 +102,26 @@ Layout make_layout(const std::vector<std::vector<int>>& in_edges, int budget_row
 }
 
 // Step C: bank classes.  cls[v] in [0, nb) for v < Nv (real nodes first, then virtual fillers so
-// that every class has exactly Nv/nb members).  Minimises sum over passes of
-// max over its groups of max(longest row, heaviest bank), ties broken by sum of squared loads.
+// that every class has exactly Nv/nb members).  Minimises the shared-memory wavefronts of a time step: per pass CG x
+// (max over its groups of max(longest row, heaviest bank)) for the gathers plus, per group, the largest number of its
+// lanes that store to the same class (every lane stores one entry per pass: its node's, or its private scratch
+// entry); ties broken by sum of squared loads.
 struct BankOpt {
   int nb, CG, n_groups;
   std::vector<int> rowmax;                          // [group]
   std::vector<std::vector<std::pair<int, int>>> feeds;   // node -> (group, #edges into it)
   std::vector<int> load;                            // [group][nb]
   std::vector<int> gcost;                           // [group]
+  std::vector<int> sgroup;                          // node -> group of the lane that stores its entry (-1: virtual filler)
+  std::vector<int> scount;                          // [group][nb] lanes of the group that store to the class
+  std::vector<int> smax;                            // [group]
   long long sumsq = 0;
+
+  int store_cost(int g) const {
+    int m = 0;
+    for (int c = 0; c < nb; ++c) m = std::max(m, scount[(size_t)g * nb + c]);
+    return m;
+  }
 
   int group_cost(int g) const {
     int m = rowmax[g];
@@ -122,11 +133,13 @@ struct BankOpt {
     for (int p = 0; p * CG < n_groups; ++p) {
       int m = 0;
       for (int g = p * CG; g < (p + 1) * CG; ++g) m = std::max(m, gcost[g]);
-      t += m;
+      t += (long long)CG * m;
+      for (int g = p * CG; g < (p + 1) * CG; ++g) t += smax[g];
     }
     return t;
   }
   void move(int v, int from, int to) {
+    if (sgroup[v] >= 0) { --scount[(size_t)sgroup[v] * nb + from]; ++scount[(size_t)sgroup[v] * nb + to]; }
     for (auto [g, cnt] : feeds[v]) {
       int& a = load[(size_t)g * nb + from];
       int& b = load[(size_t)g * nb + to];
@@ -137,7 +150,7 @@ struct BankOpt {
   }
 };
 
-std::vector<int> assign_classes(const Layout& lay, const int32_t* edge_src, int N, int CG, bool optimise,
+std::vector<int> assign_classes(const Layout& lay, const int32_t* edge_src, int N, int CG, bool optimise, bool count_stores,
                                 std::vector<int>* pass_iters) {
   const int nb = 32 / CG;
   const int n_pass = (int)lay.passes.size();
@@ -146,6 +159,16 @@ std::vector<int> assign_classes(const Layout& lay, const int32_t* edge_src, int 
   bo.rowmax.assign(bo.n_groups, 0);
   const int per_class = (N + nb - 1) / nb, Nv = per_class * nb;
   bo.feeds.assign(Nv, {});
+  bo.sgroup.assign(Nv, -1);
+  bo.scount.assign((size_t)bo.n_groups * nb, 0);
+  for (int p = 0; p < n_pass; ++p)
+    for (int l = 0; l < 32; ++l) {
+      const Row& r = lay.passes[p][l];
+      const int g = p * CG + l / nb;
+      if (!count_stores) continue;
+      if (r.node >= 0 && r.head) bo.sgroup[r.node] = g;
+      else ++bo.scount[(size_t)g * nb + l % nb];      // scratch entry of lane l: class l mod nb
+    }
   std::vector<int> outdeg(N, 0);
   {
     std::vector<std::vector<int>> cnt(bo.n_groups);   // sources feeding each group
@@ -177,6 +200,10 @@ std::vector<int> assign_classes(const Layout& lay, const int32_t* edge_src, int 
   bo.load.assign((size_t)bo.n_groups * nb, 0);
   for (int v = 0; v < N; ++v)
     for (auto [g, cnt] : bo.feeds[v]) bo.load[(size_t)g * nb + cls[v]] += cnt;
+  for (int v = 0; v < N; ++v)
+    if (bo.sgroup[v] >= 0) ++bo.scount[(size_t)bo.sgroup[v] * nb + cls[v]];
+  bo.smax.resize(bo.n_groups);
+  for (int g = 0; g < bo.n_groups; ++g) bo.smax[g] = bo.store_cost(g);
   bo.sumsq = 0;
   for (int x : bo.load) bo.sumsq += (long long)x * x;
   bo.gcost.resize(bo.n_groups);
@@ -199,6 +226,10 @@ std::vector<int> assign_classes(const Layout& lay, const int32_t* edge_src, int 
       old.resize(touched.size());
       for (size_t k = 0; k < touched.size(); ++k) old[k] = bo.gcost[touched[k]];
       for (size_t k = 0; k < touched.size(); ++k) bo.gcost[touched[k]] = bo.group_cost(touched[k]);
+      const int sga = bo.sgroup[a], sgb = bo.sgroup[b];
+      const int olda = sga >= 0 ? bo.smax[sga] : 0, oldb = sgb >= 0 ? bo.smax[sgb] : 0;
+      if (sga >= 0) bo.smax[sga] = bo.store_cost(sga);
+      if (sgb >= 0) bo.smax[sgb] = bo.store_cost(sgb);
       const long long p = bo.primary();
       if (p < best_p || (p == best_p && bo.sumsq <= best_s)) {
         best_p = p; best_s = bo.sumsq;
@@ -207,6 +238,8 @@ std::vector<int> assign_classes(const Layout& lay, const int32_t* edge_src, int 
         bo.move(a, cb, ca);
         bo.move(b, ca, cb);
         for (size_t k = touched.size(); k-- > 0;) bo.gcost[touched[k]] = old[k];
+        if (sga >= 0) bo.smax[sga] = olda;
+        if (sgb >= 0) bo.smax[sgb] = oldb;
       }
     }
   }
@@ -276,6 +309,7 @@ PlanOptions PlanOptions::from_env() {
   PlanOptions o;
   if (const char* e = tsa::tune_env("TSA_NO_SPLIT")) o.split_rows = !(e[0] == '1');
   if (const char* e = tsa::tune_env("TSA_NO_BANKOPT")) o.bank_opt = !(e[0] == '1');
+  if (const char* e = tsa::tune_env("TSA_NO_STOREOPT")) o.store_opt = !(e[0] == '1');
   if (const char* e = tsa::tune_env("TSA_NO_TIERS")) o.tiers = !(e[0] == '1');
   if (const char* e = tsa::tune_env("TSA_TEAM_MIN")) o.min_team_warps = std::max(1, std::atoi(e));
   if (const char* e = tsa::tune_env("TSA_MAX_SLOTS")) o.max_lane_slots = std::max(0, std::atoi(e));
@@ -366,7 +400,7 @@ int build_plan(const sa_network* net, const sa_observations* obs, bool need_obs,
   for (int c : cand) {
     Layout lay = make_layout(in_edges, 32 * c, opt.split_rows);
     std::vector<int> iters;
-    std::vector<int> cls = assign_classes(lay, net->edge_src, N, CG, opt.bank_opt, &iters);
+    std::vector<int> cls = assign_classes(lay, net->edge_src, N, CG, opt.bank_opt, opt.store_opt, &iters);
     const double cost = layout_cost(lay, iters);
     if (cost < best_cost) { best_cost = cost; best_lay = std::move(lay); best_cls = std::move(cls); best_iters = std::move(iters); }
   }

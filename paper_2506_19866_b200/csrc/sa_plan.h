@@ -14,6 +14,7 @@ namespace tsa {
 struct PlanOptions {
   bool split_rows = true;     // split long rows over consecutive lanes (TSA_NO_SPLIT=1 disables)
   bool bank_opt = true;       // optimise bank classes by hill climbing (TSA_NO_BANKOPT=1 disables)
+  bool store_opt = true;      // ... counting the conflicts of the result stores too (TSA_NO_STOREOPT=1: gathers only)
   bool tiers = true;          // group the passes into tiers for the statically scheduled kernel (TSA_NO_TIERS=1 disables)
   int min_team_warps = 1;     // lower bound of warps per chain (few chains: spread each over more warps)
   int max_lane_slots = 0;     // edge slots one thread may hold in registers; 0 = default for the CG
