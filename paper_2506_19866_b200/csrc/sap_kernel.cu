@@ -194,10 +194,11 @@ __device__ __forceinline__ void transition(const Lane& L, u32 t, const u32* cost
   u32 top = 0u;
   Images<0, RB>::run(L, t, s, last, cnt, tg, pr, top);
   top = group_max(top);
+  top = top != 0u ? top : 0xFFFFFFFFu;                                // nobody eligible: no priority equals it
 #pragma unroll
   for (int n = 0; n < NS; ++n) {
     const int delta = (int)tg[n] - (int)s[n];
-    const bool mv = pr[n] == top && pr[n] != 0u;                      // the nodes sharing the highest priority (:82)
+    const bool mv = pr[n] == top;                                     // the nodes sharing the highest priority (:82)
     const int step = min(max(delta, -L.d[n]), L.d[n]);                // at most d_i levels toward K_i (:80)
     s[n] = (u32)((int)s[n] + (mv ? step : 0));
     last[n] = mv ? t : last[n];
