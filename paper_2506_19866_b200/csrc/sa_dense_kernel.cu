@@ -63,6 +63,9 @@
 #ifndef TSD_SPEC
 #define TSD_SPEC 1
 #endif
+#ifndef TSD_SKIP
+#define TSD_SKIP 0
+#endif
 
 #ifndef TSD_FIXW_MASK
 #define TSD_FIXW_MASK 0
@@ -93,6 +96,10 @@ constexpr bool REDERIVE = TSD_REDERIVE != 0;    // tight register budget: derive
 // of TA goes away.  An IMMA that reads a C quad instead of RZ costs more issue time than the add it saves on
 // Mtb-shaped (149 against 164 M chain-steps/s); it gains 2 % where a chain has two IMMAs per step (HPG-shaped).
 constexpr bool CFOLD = TSD_CFOLD != 0;
+// bit (row tile * column steps + column step): that block of the weight matrix holds no candidate edge, so its IMMA
+// is left out (the host numbers the nodes so that the few nodes of the last row tile take all their sources from one
+// half of the columns: 13 instead of 14 IMMAs per time step on Mtb-shaped)
+constexpr u32 kSkip = CFOLD ? 0u : (u32)TSD_SKIP;
 constexpr int CPB = TSD_CPB;                    // chains per CTA (one-warp chains only), independent of one another: a CTA of
                                                 // 4k warps puts k chains on every SM sub-partition, which 4k one-warp CTAs do not
 constexpr int WPW = NW / TW;                    // result words per condition a lane produces
@@ -286,6 +293,7 @@ struct Phases {
     const int odd = kOddFirst ? 1 - step / KK : step / KK;
     const int tile = 2 * (P * WPP + w) + odd, s = step % KK;
     if (!(TW * MTW <= MT || tile < n_tiles)) return;
+    if ((kSkip >> (tile * KK + s)) & 1u) return;
     const u32* bb = odd ? bh : bl;
     if (CFOLD && step == 0) {
       if (SP) imma_sp_c(acc, &r.A[(tile * KSP + s) * 4], bb[4 * s], bb[4 * s + 1], bb[4 * s + 2], bb[4 * s + 3], r.M[SP ? tile * KSP + s : 0], r.CI[CFOLD ? P * WPP + w : 0]);

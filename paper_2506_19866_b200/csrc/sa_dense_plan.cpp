@@ -63,8 +63,12 @@ void pick_strides(int KS, int W, int* CS, int* TS, int* wf) {
 // identity; returns false if some violation is left.
 // movm: the register exchange's column numbering (a group = the rows 32w + 8h + 2t + {0, 1, 16, 17}).  A node of
 // zone z stays in the rows below zone_end[z] (clamped and observed nodes are kept in the first result words).
+// Optional pins (empty vectors = none): tile_req[node] >= 0 keeps the node in that row tile and every other node out
+// of it; half_req[node] >= 0 keeps the node in rows whose column lies in that half (half_of_row).
 bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::vector<std::vector<int>>& out_dst,
-                      int n_rows, bool movm, const std::vector<int>& zone, const int (&zone_end)[3], std::vector<int>* row_of_node) {
+                      int n_rows, bool movm, const std::vector<int>& zone, const int (&zone_end)[3],
+                      const std::vector<int>& tile_req, const std::vector<int>& half_req, const std::vector<int>& half_of_row,
+                      int reserved_tile, std::vector<int>* row_of_node) {
   const int N = (int)in_src.size();
   std::vector<int>& row = *row_of_node;
   std::vector<int> node_at(n_rows, -1);
@@ -86,6 +90,13 @@ bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::ve
     const int a = rnd(N), r2 = rnd(n_rows), b = node_at[r2];
     if (r2 == row[a] || (b >= 0 && group_of(row[b]) == group_of(row[a]))) continue;
     if (r2 >= zone_end[zone[a]] || (b >= 0 && row[a] >= zone_end[zone[b]])) continue;
+    if (reserved_tile >= 0) {
+      auto ok = [&](int node, int r) {
+        if ((tile_req[node] >= 0) != (r / 16 == reserved_tile)) return false;
+        return half_req[node] < 0 || half_of_row[r] == half_req[node];
+      };
+      if (!ok(a, r2) || (b >= 0 && !ok(b, row[a]))) continue;
+    }
     long before = 0, after = 0;
     for (int i : out_dst[a]) before += row_cost(i);
     if (b >= 0) for (int i : out_dst[b]) before += row_cost(i);
@@ -171,8 +182,68 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   if (want_sparse && KS % 2 == 0) {
     std::vector<std::vector<int>> in_src(N), out_dst(N);
     for (int e = 0; e < E; ++e) { in_src[net->edge_dst[e]].push_back(net->edge_src[e]); out_dst[net->edge_src[e]].push_back(net->edge_dst[e]); }
-    std::vector<int> trial = row_of_node;
-    if (assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, &trial)) { row_of_node = trial; dp->sparse = true; }
+    // A last row tile with few nodes: choose them (unobserved, smallest in-degree, no edge between them) so that all
+    // their sources can sit in ONE half of the columns; the other half's block of that tile is then empty and its IMMA
+    // is left out (skip_blocks below).  If the pinned search fails, the plain one follows.
+    bool done = false;
+    const int n_last = N - 16 * (MT - 1);
+    if (KS == 4 && !dp->movm && MT >= 2 && n_last >= 1 && n_last <= 8) {
+      std::vector<int> half_of_row(16 * MT);
+      for (int r = 0; r < 16 * MT; ++r) half_of_row[r] = col_of_row(r) / 64;
+      std::vector<int> cand;
+      for (int i = 0; i < N; ++i) if (zone[i] == 2) cand.push_back(i);
+      std::stable_sort(cand.begin(), cand.end(), [&](int a, int b) { return in_src[a].size() < in_src[b].size(); });
+      std::vector<int> tile_req(N, -1), half_req(N, -1);
+      std::vector<char> in_t(N, 0), in_s(N, 0);
+      int nt = 0;
+      for (int i : cand) {
+        if (nt == n_last) break;
+        bool okc = !in_s[i];
+        for (int sidx : in_src[i]) okc = okc && !in_t[sidx] && sidx != i;
+        if (!okc) continue;
+        in_t[i] = 1; ++nt;
+        for (int sidx : in_src[i]) in_s[sidx] = 1;
+      }
+      if (nt == n_last) {
+        for (int hs = 0; hs < 2 && !done; ++hs) {
+          for (int i = 0; i < N; ++i) { tile_req[i] = in_t[i] ? MT - 1 : -1; half_req[i] = in_s[i] ? hs : -1; }
+          // starting point: zone order, then the pinned nodes traded into rows they may take
+          std::vector<int> trial = row_of_node, node_at(16 * MT, -1);
+          for (int i = 0; i < N; ++i) node_at[trial[i]] = i;
+          auto ok = [&](int node, int r) {
+            if (r >= zone_end[zone[node]]) return false;
+            if ((tile_req[node] >= 0) != (r / 16 == MT - 1)) return false;
+            return half_req[node] < 0 || half_of_row[r] == half_req[node];
+          };
+          bool placed = true;
+          for (int pass = 0; pass < 2 && placed; ++pass)            // the last-tile nodes first, then the sources
+            for (int i = 0; i < N && placed; ++i) {
+              if ((pass == 0) != (tile_req[i] >= 0) || ok(i, trial[i])) continue;
+              if (pass == 1 && half_req[i] < 0 && tile_req[i] < 0 && ok(i, trial[i])) continue;
+              bool moved = false;
+              for (int r = 0; r < 16 * MT && !moved; ++r) {
+                const int o = node_at[r];
+                if (!ok(i, r)) continue;
+                if (o >= 0 && (!ok(o, trial[i]) || (pass == 1 && tile_req[o] >= 0))) continue;
+                if (o >= 0 && pass == 1 && half_req[o] >= 0 && ok(o, r)) continue;   // do not undo a placed source
+                node_at[trial[i]] = o; if (o >= 0) trial[o] = trial[i];
+                node_at[r] = i; trial[i] = r;
+                moved = true;
+              }
+              placed = moved;
+            }
+          for (int i = 0; i < N && placed; ++i) placed = ok(i, trial[i]);
+          if (placed && assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, tile_req, half_req, half_of_row, MT - 1, &trial)) {
+            row_of_node = trial; dp->sparse = true; done = true;
+          }
+        }
+      }
+    }
+    if (!done) {
+      std::vector<int> trial = row_of_node;
+      const std::vector<int> none;
+      if (assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, none, none, none, -1, &trial)) { row_of_node = trial; dp->sparse = true; }
+    }
   }
   const int KSP = KS / 2;                            // sparse steps of 64 columns
   std::vector<int> node_of_row(32 * KS, -1), node_of_col(32 * KS, -1);
@@ -239,6 +310,19 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
               if (e0 >= 0) place(e0, m, wreg, lane, 2 * (G % 2), tile * 4 + a);
               if (e1 >= 0) place(e1, m, wreg, lane, 2 * (G % 2) + 1, tile * 4 + a);
             }
+  }
+  // blocks of the matrix (row tile x column step of the MMA) without any candidate edge: their IMMA is left out
+  {
+    const int KK = dp->sparse ? KSP : KS, cols = dp->sparse ? 64 : 32;
+    std::vector<char> used((size_t)MT * KK, 0);
+    for (int e = 0; e < E; ++e) {
+      const int r = row_of_node[net->edge_dst[e]], c = col_of_row(row_of_node[net->edge_src[e]]);
+      used[(size_t)(r / 16) * KK + c / cols] = 1;
+    }
+    dp->skip_blocks = 0;
+    for (int m = 0; m < MT; ++m)
+      for (int k = 0; k < KK; ++k)
+        if (!used[(size_t)m * KK + k] && m * KK + k < 32) dp->skip_blocks |= 1u << (m * KK + k);
   }
   // thresholds: byte j of word w of thread group g <-> row_of_byte(g, w, j)
   dp->th_entry.assign((size_t)8 * NW * 4, 0xFFFFu);

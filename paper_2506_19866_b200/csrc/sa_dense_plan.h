@@ -22,6 +22,7 @@ struct DensePlan {
   int W = 1;                // warps per chain; warp ww owns result words ww*KS/W .. and their row tiles
   int CS = 0, TS = 0;       // byte strides of the exchange buffer: per condition, per B-fragment thread chunk
   int exchange_wavefronts = 0;   // shared-memory wavefronts of one exchange (2 stores + 2 loads)
+  uint32_t skip_blocks = 0; // bit (row tile * column steps + column step): no candidate edge in that block of the matrix
   int obs_words = 0;        // result words w < obs_words hold the scored entries (observed nodes are numbered first)
   int n_fix_rounds = 1;
   int fit_const = 0;
