@@ -303,7 +303,7 @@ def run_ours(args) -> dict:
              "peak_source": f"{sms} SMs x 4 schedulers x {sm_hz/1e6:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §7)",
              "kernel": kn, "kernel_ms": kernel_s * 1e3,
              # HBM traffic of the launch is the stage + write-back of the chains (2P + 8 bytes per chain each way,
-             # ~6 MB per launch in profiles/r2c_mtb_dense.md); it is not re-measured in this run
+             # ~6 MB per launch in profiles/r2d_mtb_dense.md); it is not re-measured in this run
              "traffic": None,
              "alg_ops_per_chain_step": prob.alg_ops_per_step,
              "useful_frac": prob.alg_ops_per_step * rate / (issue_peak * 32)}
@@ -326,7 +326,7 @@ def run_ours(args) -> dict:
             # second ceiling of the dense kernel: MMA instructions per time step against the rate of the
             # legacy tensor path measured in this run (sa_imma_peak)
             di = m["info"]["dense"]
-            per_step = prob.n_steps * di["row_tiles"] * (di["col_steps"] // 2 if di["sparse"] else di["col_steps"])
+            per_step = prob.n_steps * di["immas_per_step"]
             peak = imma["imma_sp_16864"] if di["sparse"] else imma["imma_16832"]
             r["tensor_pipe"] = {"imma_per_chain_step": per_step, "sparse_2of4": bool(di["sparse"]),
                                 "achieved_imma_per_s": per_step * rate, "peak_imma_per_s": peak,

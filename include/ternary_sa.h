@@ -163,7 +163,8 @@ int sa_get_info(sa_handle *h, int64_t info[16]);
  * tiles MT, [2] = 32-column steps KS, [3] = 1 if the 2:4-sparse A operand is used (mma.sp m16n8k64:
  * MT * KS/2 IMMAs per time step instead of MT * KS), [4] = warps per chain, [5] = resident CTAs per
  * SM of the loaded kernel (0 before the first sa_run), [6] = chain-steps per slot of the last sa_run
- * if it used balanced slots (else 0), [7] = shared-memory wavefronts of one state exchange. */
+ * if it used balanced slots (else 0), [7] = IMMAs per simulated time step (the blocks of the matrix that hold a
+ * candidate edge: MT * KS/2 or MT * KS minus the empty ones). */
 int sa_get_dense_info(sa_handle *h, int64_t info[8]);
 
 /* Kernel family of sa_run.  AUTO (default): the dense kernel — the node update as an int8 product

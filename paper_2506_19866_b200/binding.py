@@ -280,7 +280,7 @@ def sa_get_info(h: int) -> dict:
 def sa_get_dense_info(h: int) -> dict:
     info = np.zeros(8, dtype=np.int64)
     _check(_lib.sa_get_dense_info(h, info.ctypes.data), "sa_get_dense_info")
-    keys = ("applies", "row_tiles", "col_steps", "sparse", "team_warps", "ctas_per_sm", "slot_steps", "exchange_wavefronts")
+    keys = ("applies", "row_tiles", "col_steps", "sparse", "team_warps", "ctas_per_sm", "slot_steps", "immas_per_step")
     return dict(zip(keys, (int(v) for v in info)))
 
 

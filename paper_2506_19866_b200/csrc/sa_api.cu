@@ -773,7 +773,12 @@ int sa_get_dense_info(sa_handle* h, int64_t info[8]) {
   info[4] = h->dplan.W;
   info[5] = h->dk ? h->dk->blocks_per_sm : 0;
   info[6] = h->last_slot_steps;
-  info[7] = h->dplan.exchange_wavefronts;
+  {
+    const int blocks = h->dplan.MT * (h->dplan.sparse ? h->dplan.KS / 2 : h->dplan.KS);
+    int skipped = 0;
+    for (int b = 0; b < blocks && b < 32; ++b) skipped += (int)((h->dplan.skip_blocks >> b) & 1u);
+    info[7] = blocks - skipped;
+  }
   return SA_OK;
 }
 
