@@ -63,12 +63,12 @@ void pick_strides(int KS, int W, int* CS, int* TS, int* wf) {
 // identity; returns false if some violation is left.
 // movm: the register exchange's column numbering (a group = the rows 32w + 8h + 2t + {0, 1, 16, 17}).  A node of
 // zone z stays in the rows below zone_end[z] (clamped and observed nodes are kept in the first result words).
-// Optional pins (empty vectors = none): tile_req[node] >= 0 keeps the node in that row tile and every other node out
-// of it; half_req[node] >= 0 keeps the node in rows whose column lies in that half (half_of_row).
+// Optional pins (empty vectors = none): tile_req[node] >= 0 keeps the node in that row tile, reserved[tile] keeps every
+// other node out of it; half_req[node] >= 0 keeps the node in rows whose column lies in that half (half_of_row).
 bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::vector<std::vector<int>>& out_dst,
                       int n_rows, bool movm, const std::vector<int>& zone, const int (&zone_end)[3],
                       const std::vector<int>& tile_req, const std::vector<int>& half_req, const std::vector<int>& half_of_row,
-                      int reserved_tile, std::vector<int>* row_of_node) {
+                      const std::vector<char>& reserved, std::vector<int>* row_of_node) {
   const int N = (int)in_src.size();
   std::vector<int>& row = *row_of_node;
   std::vector<int> node_at(n_rows, -1);
@@ -90,9 +90,9 @@ bool assign_rows_2of4(const std::vector<std::vector<int>>& in_src, const std::ve
     const int a = rnd(N), r2 = rnd(n_rows), b = node_at[r2];
     if (r2 == row[a] || (b >= 0 && group_of(row[b]) == group_of(row[a]))) continue;
     if (r2 >= zone_end[zone[a]] || (b >= 0 && row[a] >= zone_end[zone[b]])) continue;
-    if (reserved_tile >= 0) {
+    if (!reserved.empty()) {
       auto ok = [&](int node, int r) {
-        if ((tile_req[node] >= 0) != (r / 16 == reserved_tile)) return false;
+        if (tile_req[node] >= 0 ? r / 16 != tile_req[node] : reserved[r / 16] != 0) return false;
         return half_req[node] < 0 || half_of_row[r] == half_req[node];
       };
       if (!ok(a, r2) || (b >= 0 && !ok(b, row[a]))) continue;
@@ -182,67 +182,92 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
   if (want_sparse && KS % 2 == 0) {
     std::vector<std::vector<int>> in_src(N), out_dst(N);
     for (int e = 0; e < E; ++e) { in_src[net->edge_dst[e]].push_back(net->edge_src[e]); out_dst[net->edge_src[e]].push_back(net->edge_dst[e]); }
-    // A last row tile with few nodes: choose them (unobserved, smallest in-degree, no edge between them) so that all
-    // their sources can sit in ONE half of the columns; the other half's block of that tile is then empty and its IMMA
-    // is left out (skip_blocks below).  If the pinned search fails, the plain one follows.
+    // Empty blocks (see skip_blocks below): a row tile whose nodes take ALL their sources from one half of the columns
+    // leaves its other block of the weight matrix without a candidate edge, and that block's IMMA is left out.
+    // T = the few nodes of the last row tile (unobserved ones of small in-degree), X = a whole tile of 16 more nodes,
+    // both chosen greedily so that the union S of their sources stays small; T and X are pinned to their tiles, S to
+    // one half of the columns, and the 2:4 search runs under those pins.  Attempts: T and X (two blocks), T alone
+    // (one), then the plain search.
     bool done = false;
     const int n_last = N - 16 * (MT - 1);
-    if (KS == 4 && !dp->movm && MT >= 2 && n_last >= 1 && n_last <= 8) {
-      std::vector<int> half_of_row(16 * MT);
-      for (int r = 0; r < 16 * MT; ++r) half_of_row[r] = col_of_row(r) / 64;
-      std::vector<int> cand;
-      for (int i = 0; i < N; ++i) if (zone[i] == 2) cand.push_back(i);
-      std::stable_sort(cand.begin(), cand.end(), [&](int a, int b) { return in_src[a].size() < in_src[b].size(); });
-      std::vector<int> tile_req(N, -1), half_req(N, -1);
-      std::vector<char> in_t(N, 0), in_s(N, 0);
-      int nt = 0;
-      for (int i : cand) {
-        if (nt == n_last) break;
-        bool okc = !in_s[i];
-        for (int sidx : in_src[i]) okc = okc && !in_t[sidx] && sidx != i;
-        if (!okc) continue;
-        in_t[i] = 1; ++nt;
-        for (int sidx : in_src[i]) in_s[sidx] = 1;
-      }
-      if (nt == n_last) {
-        for (int hs = 0; hs < 2 && !done; ++hs) {
-          for (int i = 0; i < N; ++i) { tile_req[i] = in_t[i] ? MT - 1 : -1; half_req[i] = in_s[i] ? hs : -1; }
-          // starting point: zone order, then the pinned nodes traded into rows they may take
-          std::vector<int> trial = row_of_node, node_at(16 * MT, -1);
-          for (int i = 0; i < N; ++i) node_at[trial[i]] = i;
-          auto ok = [&](int node, int r) {
-            if (r >= zone_end[zone[node]]) return false;
-            if ((tile_req[node] >= 0) != (r / 16 == MT - 1)) return false;
-            return half_req[node] < 0 || half_of_row[r] == half_req[node];
-          };
-          bool placed = true;
-          for (int pass = 0; pass < 2 && placed; ++pass)            // the last-tile nodes first, then the sources
-            for (int i = 0; i < N && placed; ++i) {
-              if ((pass == 0) != (tile_req[i] >= 0) || ok(i, trial[i])) continue;
-              if (pass == 1 && half_req[i] < 0 && tile_req[i] < 0 && ok(i, trial[i])) continue;
-              bool moved = false;
-              for (int r = 0; r < 16 * MT && !moved; ++r) {
-                const int o = node_at[r];
-                if (!ok(i, r)) continue;
-                if (o >= 0 && (!ok(o, trial[i]) || (pass == 1 && tile_req[o] >= 0))) continue;
-                if (o >= 0 && pass == 1 && half_req[o] >= 0 && ok(o, r)) continue;   // do not undo a placed source
-                node_at[trial[i]] = o; if (o >= 0) trial[o] = trial[i];
-                node_at[r] = i; trial[i] = r;
-                moved = true;
-              }
-              placed = moved;
-            }
-          for (int i = 0; i < N && placed; ++i) placed = ok(i, trial[i]);
-          if (placed && assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, tile_req, half_req, half_of_row, MT - 1, &trial)) {
-            row_of_node = trial; dp->sparse = true; done = true;
+    if (KS == 4 && !dp->movm && MT >= 3 && n_last >= 1 && n_last <= 8) {
+      const int n_rows = 16 * MT;
+      std::vector<int> half_of_row(n_rows);
+      for (int r = 0; r < n_rows; ++r) half_of_row[r] = col_of_row(r) / 64;
+      std::vector<std::vector<char>> src_of(N, std::vector<char>(N, 0));
+      for (int i = 0; i < N; ++i) for (int sidx : in_src[i]) src_of[i][sidx] = 1;
+      // greedy: add the node that enlarges the union of sources least (ties: smaller in-degree, lower index)
+      auto grow = [&](std::vector<char>& chosen, std::vector<char>& uni, int count, bool zone2_only) {
+        for (int k = 0; k < count; ++k) {
+          int best = -1, best_u = 1 << 30;
+          for (int i = 0; i < N; ++i) {
+            if (chosen[i] || (zone2_only && zone[i] != 2)) continue;
+            int u = 0;
+            for (int j = 0; j < N; ++j) u += (uni[j] || src_of[i][j]) ? 1 : 0;
+            if (u < best_u || (u == best_u && in_src[i].size() < in_src[best].size())) { best_u = u; best = i; }
           }
+          if (best < 0) return false;
+          chosen[best] = 1;
+          for (int j = 0; j < N; ++j) uni[j] = uni[j] || src_of[best][j];
+        }
+        return true;
+      };
+      auto attempt = [&](const std::vector<int>& tile_req, const std::vector<int>& half_req, const std::vector<char>& reserved) {
+        // constructive start: zone by zone, the pinned nodes first, the free ones preferably in the other half
+        std::vector<int> trial(N, -1), node_at(n_rows, -1);
+        auto put = [&](int node, int want_half, bool strict) {
+          for (int r = 0; r < n_rows; ++r) {
+            if (node_at[r] >= 0 || r >= zone_end[zone[node]]) continue;
+            if (tile_req[node] >= 0 ? r / 16 != tile_req[node] : reserved[r / 16] != 0) continue;
+            if (strict && want_half >= 0 && half_of_row[r] != want_half) continue;
+            node_at[r] = node; trial[node] = r;
+            return true;
+          }
+          return false;
+        };
+        int hs = -1;
+        for (int i = 0; i < N; ++i) if (half_req[i] >= 0) hs = half_req[i];
+        for (int z = 0; z < 3; ++z) {
+          for (int i = 0; i < N; ++i) if (zone[i] == z && tile_req[i] >= 0 && !put(i, half_req[i], true)) return false;
+          for (int i = 0; i < N; ++i) if (zone[i] == z && tile_req[i] < 0 && half_req[i] >= 0 && !put(i, half_req[i], true)) return false;
+          for (int i = 0; i < N; ++i)
+            if (zone[i] == z && tile_req[i] < 0 && half_req[i] < 0 && !put(i, 1 - hs, hs >= 0) && !put(i, -1, false)) return false;
+        }
+        if (!assign_rows_2of4(in_src, out_dst, n_rows, dp->movm, zone, zone_end, tile_req, half_req, half_of_row, reserved, &trial)) return false;
+        row_of_node = trial;
+        return true;
+      };
+      std::vector<char> in_t(N, 0), uni_t(N, 0);
+      const bool have_t = grow(in_t, uni_t, n_last, true);
+      for (int variant = 0; variant < 2 && have_t && !done; ++variant) {          // 0: T and X, 1: T alone
+        std::vector<char> chosen = in_t, uni = uni_t;
+        int x_tile = -1;
+        if (variant == 0) {
+          if (!grow(chosen, uni, 16, false)) continue;
+          bool x_observed = false;
+          for (int i = 0; i < N; ++i) x_observed = x_observed || (chosen[i] && !in_t[i] && zone[i] != 2);
+          x_tile = x_observed ? zone_end[1] / 16 - 1 : MT - 2;
+          if (x_tile < 0 || x_tile >= MT - 1) continue;
+        }
+        for (int hs = 0; hs < 2 && !done; ++hs) {
+          std::vector<int> tile_req(N, -1), half_req(N, -1);
+          std::vector<char> reserved(MT, 0);
+          reserved[MT - 1] = 1;
+          if (x_tile >= 0) reserved[x_tile] = 1;
+          for (int i = 0; i < N; ++i) {
+            if (in_t[i]) tile_req[i] = MT - 1;
+            else if (chosen[i]) tile_req[i] = x_tile;
+            if (uni[i]) half_req[i] = hs;
+          }
+          done = attempt(tile_req, half_req, reserved);
         }
       }
+      if (done) dp->sparse = true;
     }
     if (!done) {
       std::vector<int> trial = row_of_node;
       const std::vector<int> none;
-      if (assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, none, none, none, -1, &trial)) { row_of_node = trial; dp->sparse = true; }
+      if (assign_rows_2of4(in_src, out_dst, 16 * MT, dp->movm, zone, zone_end, none, none, none, std::vector<char>(), &trial)) { row_of_node = trial; dp->sparse = true; }
     }
   }
   const int KSP = KS / 2;                            // sparse steps of 64 columns
