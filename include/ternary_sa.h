@@ -195,7 +195,8 @@ int sa_select_kernel(sa_handle *h, int family);
 /* Host only (no GPU needed): build the plan of a problem for n_chains chains and compile the
  * statically scheduled kernel for it.  info[0] = 1 if the static kernel applies, [1] = warps per
  * chain, [2] = tiers, [3] = edge slots per thread, [4] = cubin bytes, [5] = shared memory bytes per
- * CTA, [6] = 1 if the dense kernel applies, [7] = its cubin bytes; log (may be NULL) receives the reason / NVRTC log, truncated to log_bytes.  Returns SA_OK
+ * CTA, [6] = 1 if the dense kernel applies, [7] = its cubin bytes; log (may be NULL) receives the reason / NVRTC log, truncated to log_bytes,
+ * or on success a line "dense plan: sparse=S immas_per_step=I obs_words=W" for the dense kernel.  Returns SA_OK
  * also when the kernel does not apply (info[0] = 0); SA_ECUDA when NVRTC is missing or fails. */
 int sa_jit_check(const sa_network *net, const sa_observations *obs, int32_t n_chains, int64_t info[8],
                  char *log, size_t log_bytes);

@@ -710,7 +710,7 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
     if (log && log_bytes) { std::strncpy(log, s.c_str(), log_bytes - 1); log[log_bytes - 1] = 0; }
   };
   tsa::Plan pl;
-  std::string err;
+  std::string err, dense_note;
   const int rc = tsa::build_plan(net, obs, obs->obs != nullptr, plan_options(n_chains, 148), &pl, &err);
   if (rc != SA_OK) return set_err(rc, err);
   {
@@ -725,9 +725,15 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
         return set_err(SA_ECUDA, "dense kernel did not compile: " + clog.substr(0, 400));
       }
       info[7] = (int64_t)cubin.size();
+      const int blocks = dp.MT * (dp.sparse ? dp.KS / 2 : dp.KS);
+      int skipped = 0;
+      for (int b = 0; b < blocks && b < 32; ++b) skipped += (int)((dp.skip_blocks >> b) & 1u);
+      dense_note = "dense plan: sparse=" + std::to_string(dp.sparse ? 1 : 0) + " immas_per_step=" + std::to_string(blocks - skipped) +
+                   " obs_words=" + std::to_string(dp.obs_words);
+      put_log(dense_note);
     }
   }
-  if (pl.team_warps <= 0) { put_log(pl.static_why); return SA_OK; }
+  if (pl.team_warps <= 0) { put_log(dense_note.empty() ? pl.static_why : dense_note + "; static kernel: " + pl.static_why); return SA_OK; }
   info[0] = 1;
   info[1] = pl.team_warps;
   info[2] = pl.n_tiers;

@@ -133,6 +133,26 @@ def test_execution_plan_is_valid_for_every_config(B, problems_cache):
     assert naive["split_nodes"] == 0 and naive["edge_iterations"] > mtb["edge_iterations"]
 
 
+def test_dense_plan_leaves_empty_blocks_out(B, problems_cache):
+    """Host only: the dense kernel's plan for Mtb-shaped uses the 2:4-sparse operand, scores two of four result
+    words and leaves two of the 14 blocks of the weight matrix without a candidate edge (12 IMMAs per time step);
+    the plan is deterministic; other shapes with a small last row tile plan and compile whether or not the pinned
+    search succeeds."""
+    import re
+    from oracle import oracle as O
+    from paper_2506_19866_b200 import problems as PB
+    a = B.sa_jit_check(problems_cache("mtb"), 4096)
+    b = B.sa_jit_check(problems_cache("mtb"), 4096)
+    assert a["dense_applies"] and a["log"] == b["log"] and a["dense_cubin_bytes"] == b["dense_cubin_bytes"]
+    m = re.search(r"sparse=(\d+) immas_per_step=(\d+) obs_words=(\d+)", a["log"])
+    assert m and (int(m.group(1)), int(m.group(2)), int(m.group(3))) == (1, 12, 2), a["log"]
+    for name, N, E, degree, seed in (("eb84", 84, 500, "powerlaw", 3), ("eb104", 104, 1500, "poisson", 2)):
+        cs = PB.ConfigSpec(name, 4000 + seed, N, E, degree, 8, 3, 16, (4, 8, 12, 16), 8, 120, max_in_degree=40)
+        info = B.sa_jit_check(PB.make_problem(name, O.simulate_fn, spec=cs, noise=0.05), 8)
+        m = re.search(r"sparse=(\d+) immas_per_step=(\d+)", info["log"])
+        assert info["dense_applies"] and m and 0 < int(m.group(2)) <= (N + 15) // 16 * 4, info["log"]
+
+
 # ------------------------------------------------------------------ the paper model (sap_*)
 @pytest.fixture(scope="module")
 def paper_hpg():

@@ -339,6 +339,30 @@ def test_sparse_operand_applies_or_falls_back(B):
             check_chains(B, hd, orc, list(range(8)), 150, B.sa_get_trace(hd.h, 8, 150))
 
 
+EMPTY_BLOCK_CASES = [("eb100a", 100, 900, "powerlaw", 7), ("eb100b", 100, 700, "poisson", 11), ("eb116", 116, 640, "poisson", 5),
+                     ("eb84", 84, 500, "powerlaw", 3), ("eb68", 68, 420, "poisson", 9), ("eb104", 104, 1500, "poisson", 2)]
+
+
+@pytest.mark.parametrize("name,N,E,degree,seed", EMPTY_BLOCK_CASES, ids=[c[0] for c in EMPTY_BLOCK_CASES])
+def test_empty_blocks_of_the_weight_matrix(B, name, N, E, degree, seed):
+    """A last row tile with few nodes: the host tries to number the nodes so that one or two blocks of the weight
+    matrix hold no candidate edge (their IMMAs are left out) and falls back to the plain numbering if the pinned
+    2:4 search fails.  Whatever it finds, the results are the oracle's."""
+    cs = PB.ConfigSpec(name, 4000 + seed, N, E, degree, 8, 3, 16, (4, 8, 12, 16), 8, 120, max_in_degree=40)
+    prob = PB.make_problem(name, O.simulate_fn, spec=cs, noise=0.05)
+    orc = O.Oracle(prob)
+    sched = PB.make_schedule(8, 120)
+    with Handle(B, prob, sched) as hd:
+        B.sa_select_kernel(hd.h, B.SA_KERNEL_DENSE)
+        B.sa_set_trace(hd.h, list(range(8)), 120)
+        B.sa_run(hd.h, 120)
+        di = B.sa_get_dense_info(hd.h)
+        blocks = di["row_tiles"] * (di["col_steps"] // 2 if di["sparse"] else di["col_steps"])
+        assert di["applies"] == 1 and 0 < di["immas_per_step"] <= blocks, di
+        check_chains(B, hd, orc, list(range(8)), 120, B.sa_get_trace(hd.h, 8, 120))
+        check_all_fitness(B, hd, orc)
+
+
 def test_dense_kernel_limits(B):
     """The dense family applies up to 128 nodes and 8 conditions; beyond that DENSE fails loudly
     and AUTO falls back to the gather kernels with identical results."""
