@@ -162,7 +162,7 @@ struct Images {
     const int img = (int)acc - 4 * EN;                                  // the image K_i (:66-68)
     tg[NI] = (u32)min(max(img, 0), 2);                                  // as far as the allowable states go (:70)
     const bool eligible = tg[NI] != s[NI] && cnt[NI] >= L.m[NI];        // told to update, memory criterion met (:79, :82)
-    pr[NI] = eligible ? L.u[NI] * (t - last[NI]) : 0u;                  // speed x time steps since last updated (:82)
+    pr[NI] = eligible ? last[NI] : 0u;                                  // speed x time steps since last updated (:82), kept as a running product
     top = max(top, pr[NI]);
     Images<NI + 1, RB>::run(L, t, s, last, cnt, tg, pr, top);
   }
@@ -201,7 +201,7 @@ __device__ __forceinline__ void transition(const Lane& L, u32 t, const u32* cost
     const bool mv = pr[n] == top;                                     // the nodes sharing the highest priority (:82)
     const int step = min(max(delta, -L.d[n]), L.d[n]);                // at most d_i levels toward K_i (:80)
     s[n] = (u32)((int)s[n] + (mv ? step : 0));
-    last[n] = mv ? t : last[n];
+    last[n] = mv ? L.u[n] : last[n] + L.u[n];                         // u x (t + 1 - time of the last change): u after a move, + u otherwise
     cnt[n] = (delta != 0 && !mv) ? cnt[n] + 1u : 0u;                  // consecutive time steps told to update without moving
     const u32 sel = kSel0 + s[n];
     sts_u8<(1 - RB) * BUF_B>(L.self[n], sel);
@@ -226,7 +226,7 @@ __device__ __forceinline__ u32 simulate(const Params& p, const Lane& L, int lig,
       load_cost(cost_row, cost);
 #pragma unroll
       for (int n = 0; n < NS; ++n) {
-        s[n] = (iw >> (2 * n)) & 3u; last[n] = 0u; cnt[n] = 0u;
+        s[n] = (iw >> (2 * n)) & 3u; last[n] = L.u[n]; cnt[n] = 0u;     // age 1 at the first transition (reading P3)
         const u32 sel = kSel0 + s[n];
         sts_u8<0>(L.self[n], sel);
         y += prmt(cost[n], sel);                                      // row t0 of S, R and G (:92-100)
