@@ -190,7 +190,8 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
     // (one), then the plain search.
     bool done = false;
     const int n_last = N - 16 * (MT - 1);
-    if (KS == 4 && !dp->movm && MT >= 3 && n_last >= 1 && n_last <= 8) {
+    const bool small_last = n_last >= 1 && n_last <= 8;       // else: X alone (one block)
+    if (KS == 4 && !dp->movm && MT >= 3) {
       const int n_rows = 16 * MT;
       std::vector<int> half_of_row(n_rows);
       for (int r = 0; r < n_rows; ++r) half_of_row[r] = col_of_row(r) / 64;
@@ -238,21 +239,21 @@ void build_dense_plan(const sa_network* net, const sa_observations* obs, const P
         return true;
       };
       std::vector<char> in_t(N, 0), uni_t(N, 0);
-      const bool have_t = grow(in_t, uni_t, n_last, true);
-      for (int variant = 0; variant < 2 && have_t && !done; ++variant) {          // 0: T and X, 1: T alone
+      const bool have_t = !small_last || grow(in_t, uni_t, n_last, true);
+      for (int variant = 0; variant < (small_last ? 2 : 1) && have_t && !done; ++variant) {   // 0: T and X (or X alone), 1: T alone
         std::vector<char> chosen = in_t, uni = uni_t;
         int x_tile = -1;
         if (variant == 0) {
           if (!grow(chosen, uni, 16, false)) continue;
           bool x_observed = false;
           for (int i = 0; i < N; ++i) x_observed = x_observed || (chosen[i] && !in_t[i] && zone[i] != 2);
-          x_tile = x_observed ? zone_end[1] / 16 - 1 : MT - 2;
-          if (x_tile < 0 || x_tile >= MT - 1) continue;
+          x_tile = x_observed ? zone_end[1] / 16 - 1 : small_last ? MT - 2 : MT - 1;
+          if (x_tile < 0 || x_tile >= (small_last ? MT - 1 : MT)) continue;
         }
         for (int hs = 0; hs < 2 && !done; ++hs) {
           std::vector<int> tile_req(N, -1), half_req(N, -1);
           std::vector<char> reserved(MT, 0);
-          reserved[MT - 1] = 1;
+          if (small_last) reserved[MT - 1] = 1;
           if (x_tile >= 0) reserved[x_tile] = 1;
           for (int i = 0; i < N; ++i) {
             if (in_t[i]) tile_req[i] = MT - 1;

@@ -340,7 +340,8 @@ def test_sparse_operand_applies_or_falls_back(B):
 
 
 EMPTY_BLOCK_CASES = [("eb100a", 100, 900, "powerlaw", 7), ("eb100b", 100, 700, "poisson", 11), ("eb116", 116, 640, "poisson", 5),
-                     ("eb84", 84, 500, "powerlaw", 3), ("eb68", 68, 420, "poisson", 9), ("eb104", 104, 1500, "poisson", 2)]
+                     ("eb84", 84, 500, "powerlaw", 3), ("eb68", 68, 420, "poisson", 9), ("eb104", 104, 1500, "poisson", 2),
+                     ("eb128", 128, 800, "powerlaw", 4), ("eb112", 112, 700, "poisson", 6), ("eb90", 90, 600, "powerlaw", 8)]
 
 
 @pytest.mark.parametrize("name,N,E,degree,seed", EMPTY_BLOCK_CASES, ids=[c[0] for c in EMPTY_BLOCK_CASES])
