@@ -120,6 +120,37 @@ int sa_simulate(const sa_network *net, const sa_observations *obs, const int8_t 
  * be at a level boundary.  Asynchronous like sa_run; the synchronisation is not traced. */
 int sa_run_levels(sa_handle *h, int64_t n_levels, int32_t group_size);
 
+/* One level synchronisation (the second half of a sa_run_levels level, Table 1 :150-155) for
+ * callers that may not allocate device memory once set-up is over.
+ *
+ * Who that is: sa_run_levels takes its winner table (one u64 per group) from cudaMalloc, or from the
+ * sa_set_allocator hooks, the first time a handle calls it.  That is no use to a program that shares
+ * the GPU with a framework which has already reserved all of its memory (the request would fail, or
+ * make that framework flush its cache), to one whose own arena is frozen after start-up, or to a
+ * service loop that cannot afford the device-wide stall cudaMalloc and cudaFree imply.  Such a
+ * caller creates its handles up front, then drives Table 1 itself:
+ *     for each level { sa_run(h, steps_per_level); sa_level_sync_static(h, group_size); }
+ * which leaves the chain store exactly as sa_run_levels(h, 1, group_size) per level would.
+ *
+ * Inputs and outputs are the handle's chain store (best / current vectors and fitnesses in device
+ * memory, allocated by sa_create).  The winner table lives in a fixed array inside the library image:
+ * SA_LEVEL_SYNC_STATIC_MAX_GROUPS u64 = 512 KiB of device memory on every GPU that loads the library,
+ * held until the process exits.  The call makes no cudaMalloc / cudaFree and uses no allocating
+ * library routine; it launches two kernels on the handle's stream and returns without waiting.
+ *
+ * - ceil(n_chains / group_size) must not exceed SA_LEVEL_SYNC_STATIC_MAX_GROUPS (group_size = 0: one
+ *   group, always fits); otherwise SA_EINVAL and nothing is launched.
+ * - The device that owns the handle must be current (SA_EINVAL otherwise).
+ * - The first call on each device looks up the array's device address (cudaGetSymbolAddress) and
+ *   keeps it; make that first call before any stream capture begins.
+ * - The array is shared by every handle and every thread of the process and keeps what the last call
+ *   left in it.  Nothing in it has to start at zero: a call writes every entry it later reads.  Two
+ *   calls whose kernels can overlap on the GPU (different streams, no dependency between them) race
+ *   on it; order them with an event or use one stream.
+ * - Unlike sa_run_levels the step counter need not sit on a level boundary. */
+#define SA_LEVEL_SYNC_STATIC_MAX_GROUPS 65536
+int sa_level_sync_static(sa_handle *h, int32_t group_size);
+
 /* One chain's current and best vectors ([E+N] each) and fitnesses.  Any output may be NULL. */
 int sa_get_chain(sa_handle *h, int32_t chain, int8_t *cur, uint32_t *cur_fit, int8_t *best, uint32_t *best_fit);
 

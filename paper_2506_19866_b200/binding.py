@@ -20,13 +20,14 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_imma_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_get_dense_info", "sa_get_level_stats",
+           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_level_sync_static", "sa_get_dense_info", "sa_get_level_stats",
            "sap_create", "sap_run", "sap_run_levels", "sap_best", "sap_destroy", "sap_eval", "sap_simulate",
            "sap_get_chain", "sap_get_fitness", "sap_set_trace", "sap_get_trace", "sap_get_level_stats", "sap_get_info",
            "sap_set_stream", "sap_jit_check")
 SAP_CONSTRAINED, SAP_LEVEL_STATS = 1, 2
 SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
 SA_CONSTRAINED, SA_LEVEL_STATS = 1, 2
+SA_LEVEL_SYNC_STATIC_MAX_GROUPS = 65536
 
 if not os.path.exists(LIB_PATH):
     raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2506_19866_b200.build` "
@@ -64,6 +65,7 @@ _lib.sa_last_error.restype = C.c_char_p
 _lib.sa_create.argtypes = [C.POINTER(_Network), C.POINTER(_Observations), C.POINTER(_Schedule), C.POINTER(C.c_void_p)]
 _lib.sa_run.argtypes = [C.c_void_p, C.c_int64]
 _lib.sa_run_levels.argtypes = [C.c_void_p, C.c_int64, C.c_int32]
+_lib.sa_level_sync_static.argtypes = [C.c_void_p, C.c_int32]
 _lib.sa_best.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
 _lib.sa_destroy.argtypes = [C.c_void_p]
 _lib.sa_destroy.restype = None
@@ -206,6 +208,12 @@ def sa_run(h: int, steps: int) -> None:
 
 def sa_run_levels(h: int, n_levels: int, group_size: int = 0) -> None:
     _check(_lib.sa_run_levels(h, n_levels, group_size), "sa_run_levels")
+
+
+def sa_level_sync_static(h: int, group_size: int = 0) -> None:
+    """One level synchronisation with no device allocation (the winner table is a fixed array in the library,
+    at most SA_LEVEL_SYNC_STATIC_MAX_GROUPS groups): for callers that cannot call cudaMalloc after set-up."""
+    _check(_lib.sa_level_sync_static(h, group_size), "sa_level_sync_static")
 
 
 def sa_best(h: int, n_params: int):

@@ -528,6 +528,25 @@ int sa_run_levels(sa_handle* h, int64_t n_levels, int32_t group_size) {
   return SA_OK;
 }
 
+int sa_level_sync_static(sa_handle* h, int32_t group_size) {
+  if (!h) return set_err(SA_EINVAL, "null handle");
+  if (group_size < 0) return set_err(SA_EINVAL, "group_size < 0");
+  const int group = (group_size == 0 || group_size > h->C.R) ? h->C.R : group_size;
+  const int64_t n_groups = ((int64_t)h->C.R + group - 1) / group;
+  if (n_groups > SA_LEVEL_SYNC_STATIC_MAX_GROUPS)
+    return set_err(SA_EINVAL, "sa_level_sync_static: " + std::to_string(n_groups) + " groups (" + std::to_string(h->C.R) +
+                                  " chains in groups of " + std::to_string(group) + ") exceed the fixed winner table of " +
+                                  std::to_string(SA_LEVEL_SYNC_STATIC_MAX_GROUPS) + " groups; use larger groups or sa_run_levels");
+  const char* why = nullptr;
+  const cudaError_t e = tsa::launch_level_sync_static(h->P, h->C, group, h->stream, &why);
+  if (e != cudaSuccess) {
+    if (why) return set_err(SA_EINVAL, std::string("sa_level_sync_static: ") + why);
+    return cuda_err(e, "sa_level_sync_static");
+  }
+  h->launches += 2;
+  return SA_OK;
+}
+
 // after a stream synchronisation: did a kernel of this handle give up a hand-over wait?
 static int check_device_error(sa_handle* h) {
   if (!h->d_err) return SA_OK;

@@ -11,6 +11,10 @@
 // Shares nothing with oracle/.
 #include "sa_kernels.h"
 
+#include <mutex>
+
+#include "../../include/ternary_sa.h"
+
 namespace tsa {
 
 // ------------------------------------------------------------------------------------------
@@ -688,6 +692,56 @@ __global__ void level_broadcast_kernel(DevChains C, int EpadA, int NpadA, int gr
 
 cudaError_t launch_level_sync(const DevProblem& P, const DevChains& C, int group, unsigned long long* win, cudaStream_t st) {
   const int n_groups = (C.R + group - 1) / group;
+  group_argmin_kernel<<<n_groups, group >= 256 ? 256 : 32, 0, st>>>(C.fit_best, C.R, group, win);
+  level_broadcast_kernel<<<C.R, 128, 0, st>>>(C, P.EpadA, P.NpadA, group, win);
+  return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// Level synchronisation for callers that cannot allocate (sa_level_sync_static).
+//
+// The winners of the groups go to this array, part of the library image, instead of a buffer from cudaMalloc: every
+// GPU that loads the library carries its 512 KiB until the process ends.  All handles and threads share it and it
+// keeps the last call's winners; group_argmin_kernel rewrites entries 0..n_groups-1 before level_broadcast_kernel
+// reads them, both on the same stream, so nothing needs clearing.  Calls that overlap on the GPU race on it.
+//
+// On the host the name g_static_win is only a stand-in for the symbol, not an address a kernel could use: the device
+// address comes from cudaGetSymbolAddress, asked once per device with that device current, and is what the kernels get.
+// ------------------------------------------------------------------------------------------
+static __device__ __align__(256) unsigned long long g_static_win[SA_LEVEL_SYNC_STATIC_MAX_GROUPS];
+
+constexpr int kMaxDevices = 64;
+static std::mutex g_static_win_mu;
+static unsigned long long* g_static_win_addr[kMaxDevices] = {};   // per device ordinal, filled on first use
+
+cudaError_t launch_level_sync_static(const DevProblem& P, const DevChains& C, int group, cudaStream_t st, const char** why) {
+  *why = nullptr;
+  const int n_groups = (C.R + group - 1) / group;
+  if (n_groups > SA_LEVEL_SYNC_STATIC_MAX_GROUPS) {
+    *why = "more groups than the fixed winner table holds";
+    return cudaErrorInvalidValue;
+  }
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  cudaPointerAttributes attr;
+  e = cudaPointerGetAttributes(&attr, C.fit_best);
+  if (e != cudaSuccess) return e;
+  if (attr.type != cudaMemoryTypeDevice || attr.device != dev || dev < 0 || dev >= kMaxDevices) {
+    *why = "the device that owns the handle's chain store is not the current device";
+    return cudaErrorInvalidValue;
+  }
+  unsigned long long* win = nullptr;
+  {
+    std::lock_guard<std::mutex> lock(g_static_win_mu);
+    if (!g_static_win_addr[dev]) {
+      void* p = nullptr;
+      e = cudaGetSymbolAddress(&p, g_static_win);     // device `dev` is current: this is ITS copy of the array
+      if (e != cudaSuccess) return e;
+      g_static_win_addr[dev] = (unsigned long long*)p;
+    }
+    win = g_static_win_addr[dev];
+  }
   group_argmin_kernel<<<n_groups, group >= 256 ? 256 : 32, 0, st>>>(C.fit_best, C.R, group, win);
   level_broadcast_kernel<<<C.R, 128, 0, st>>>(C, P.EpadA, P.NpadA, group, win);
   return cudaGetLastError();

@@ -22,6 +22,10 @@ cudaError_t launch_eval(const DevProblem& P, const int8_t* w, const int8_t* th, 
 // d_best (ties: smallest chain) gives its best vector to every member as best and current vector.
 // win = device scratch, one u64 per group.
 cudaError_t launch_level_sync(const DevProblem& P, const DevChains& C, int group, unsigned long long* win, cudaStream_t st);
+// The same synchronisation with the winners kept in a fixed device array of this library instead of a buffer the
+// caller allocated (sa_level_sync_static in include/ternary_sa.h): nothing is allocated.  Returns cudaErrorInvalidValue
+// with *why set when there are more groups than the array holds or the chain store is not on the current device.
+cudaError_t launch_level_sync_static(const DevProblem& P, const DevChains& C, int group, cudaStream_t st, const char** why);
 // out[0] = (fitness << 32) | chain of the best chain (smallest fitness, then smallest index)
 cudaError_t launch_argmin(const uint32_t* fit, int R, unsigned long long* out, cudaStream_t st);
 
