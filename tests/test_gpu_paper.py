@@ -335,3 +335,58 @@ def test_source_node_and_validation(B):
             B.sap_eval(hd.h, bad)
     with pytest.raises(B.SaError):
         B.sap_create(prob, sched, B.SAP_CONSTRAINED)
+
+
+# ------------------------------------------------- the geometry the paper_mtb throughput is measured on
+# From R >= 4736 the planner gives paper_mtb 16 lanes per chain: two chains per warp, four node slots per lane
+# (sap_plan.cpp).  The long-trace tests above run the 32-lane geometry, so this one gets its own: forced at a small R,
+# then chosen by the planner at the benchmark's R, odd and even chains (the second and the first chain of a warp).
+@pytest.mark.parametrize("flags", [0, 1])
+def test_paper_mtb_two_chains_per_warp_forced(B, paper_problems, flags):
+    prob = paper_problems("paper_mtb")
+    orc = OP.PaperOracle(prob)
+    R = 601                                                   # odd: the last warp carries one chain only
+    sched = PB.paper_schedule(R, 20, 100, prob.max_objective)
+    chains = sorted(set(list(range(0, R, 29)) + list(range(1, R, 31)) + [2, 3, R - 2, R - 1]))
+    assert len(chains) >= 40 and sum(c & 1 for c in chains) >= 15 and sum(1 - (c & 1) for c in chains) >= 15
+    os.environ["TSA_PAPER_LPC"] = "16"
+    try:
+        with Handle(B, prob, sched, flags) as hd:
+            assert B.sap_get_info(hd.h)["lanes_per_chain"] == 16
+            B.sap_set_trace(hd.h, chains, 2000)
+            B.sap_run(hd.h, 700)
+            B.sap_run(hd.h, 1300)
+            check_chains(B, hd, orc, chains, 2000, B.sap_get_trace(hd.h, len(chains), 2000))
+            check_all_fitness(B, hd, orc)
+    finally:
+        del os.environ["TSA_PAPER_LPC"]
+
+
+@pytest.mark.parametrize("flags", [0, 1])
+def test_paper_mtb_benchmarked_geometry_full_length(B, paper_problems, flags):
+    prob = paper_problems("paper_mtb")
+    orc = OP.PaperOracle(prob)
+    spec = PB.PAPER_CONFIGS["paper_mtb"]
+    R, steps = spec.n_chains, spec.sa_steps                   # 10 240 chains x 5000 steps, as bench.py runs it
+    sched = PB.paper_schedule(R, 50, steps // 50, prob.max_objective)
+    chains = sorted(set(list(range(0, R, 331)) + list(range(1, R, 641)) + [R - 2, R - 1]))
+    assert len(chains) >= 32 and sum(c & 1 for c in chains) >= 10
+    with Handle(B, prob, sched, flags) as hd:
+        assert B.sap_get_info(hd.h)["lanes_per_chain"] == 16  # the planner's own choice at this R
+        B.sap_set_trace(hd.h, chains, steps)
+        B.sap_run(hd.h, 12)
+        check_chains(B, hd, orc, list(range(R)), 12)          # every chain, not every 16th
+        B.sap_run(hd.h, steps - 12)
+        check_chains(B, hd, orc, chains, steps, B.sap_get_trace(hd.h, len(chains), steps))
+        check_all_fitness(B, hd, orc)
+
+
+def test_paper_mtb_hundred_thousand_chains(B, paper_problems):
+    prob = paper_problems("paper_mtb")
+    orc = OP.PaperOracle(prob)
+    R = 102400
+    sched = PB.paper_schedule(R, 4, 5, prob.max_objective)
+    with Handle(B, prob, sched, 1) as hd:
+        assert B.sap_get_info(hd.h)["lanes_per_chain"] == 16
+        B.sap_run(hd.h, 20)
+        check_chains(B, hd, orc, list(range(0, R, 7)) + [R - 1], 20)
