@@ -334,9 +334,10 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
   // structural constraints (readings C1, C2): per node the number of non-zero in-edges,
   // non-zero out-edges and +1 in-edges of the chain's current vector, kept in shared memory behind the reduction
   // words; only the thread that holds the proposed weight reads or writes them, between two team barriers
-  unsigned char* const cin = (unsigned char*)(red + W);
-  unsigned char* const cout = cin + TSA_NN;
-  unsigned char* const cact = cout + TSA_NN;
+  // (16-bit counters: a node's out-degree is bounded by N - 1 < 65 536 only, a hub may feed more than 255 nodes)
+  unsigned short* const cin = (unsigned short*)(red + W);
+  unsigned short* const cout = cin + TSA_NN;
+  unsigned short* const cact = cout + TSA_NN;
   if (TSA_CONSTRAINED) {
     for (int i = threadIdx.x; i < TSA_NN; i += TEAM) {
       int a = 0, b = 0, c = 0;
@@ -345,7 +346,7 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
         a += v != 0; c += v == 1;
       }
       for (int x = __ldg(p.con_out_ptr + i); x < __ldg(p.con_out_ptr + i + 1); ++x) b += cur_w[__ldg(p.con_out_slot + x)] != 0;
-      cin[i] = (unsigned char)a; cout[i] = (unsigned char)b; cact[i] = (unsigned char)c;
+      cin[i] = (unsigned short)a; cout[i] = (unsigned short)b; cact[i] = (unsigned short)c;
     }
   }
 
@@ -418,8 +419,8 @@ extern "C" __global__ void __launch_bounds__(TEAM, TSA_MINBLOCKS) tsa_run_static
     if (acc) {
       fcur = fcand;
       if (TSA_CONSTRAINED && mine && is_w) {
-        cin[cdst] = (unsigned char)(cin[cdst] + dnz); cout[csrc] = (unsigned char)(cout[csrc] + dnz);
-        cact[cdst] = (unsigned char)(cact[cdst] + dact);
+        cin[cdst] = (unsigned short)(cin[cdst] + dnz); cout[csrc] = (unsigned short)(cout[csrc] + dnz);
+        cact[cdst] = (unsigned short)(cact[cdst] + dact);
       }
       if (fcand < fbest) {
         fbest = fcand;

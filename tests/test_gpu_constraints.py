@@ -122,3 +122,65 @@ def test_large_constrained_on_the_static_kernel_and_refusals(B, problems_cache):
         check(B, hd, orc, list(range(6)), 60, B.sa_get_trace(hd.h, 6, 60))
     with pytest.raises(B.SaError):                                        # tiny has nodes without in-edges
         B.sa_create(problems_cache("tiny"), PB.default_schedule("tiny"), flags=B.SA_CONSTRAINED)
+
+
+def hub_problem(n=800, hub_out=375, extra=2400, seed=77):
+    """A network whose node 0 feeds `hub_out` other nodes, on a ring that gives every node an in- and an out-edge:
+    enough of the hub's out-edges are non-zero in a repaired random vector for the count to pass through 257, so a
+    per-node counter kept in one byte would wrap (257 reads as 1) and strike moves the oracle allows."""
+    rng = np.random.default_rng(seed)
+    edges = {(i, (i + 1) % n) for i in range(n)}
+    edges |= {(0, int(d)) for d in rng.choice(np.arange(2, n), size=hub_out - 1, replace=False)}
+    while len(edges) < n + hub_out - 1 + extra:
+        s, d = (int(v) for v in rng.integers(1, n, size=2))
+        if s != d:
+            edges.add((s, d))
+    edges = sorted(edges)
+    src = np.array([e[0] for e in edges], dtype=np.int32)
+    dst = np.array([e[1] for e in edges], dtype=np.int32)
+    K, T = 4, 12
+    times = np.array([4, 8, 12], dtype=np.int32)
+    init = rng.integers(0, 3, size=(K, n)).astype(np.uint8)
+    clamp = np.zeros((K, n), dtype=np.uint8)
+    clamp[:, 5] = 1
+    prob = PB.Problem(name="hub", seed=seed, n_nodes=n, n_edges=len(edges), edge_src=src, edge_dst=dst,
+                      th_lo=np.array(PB.TH_LO, dtype=np.int8), th_hi=np.array(PB.TH_HI, dtype=np.int8), n_cond=K, n_steps=T,
+                      obs_times=times, init_state=init, clamp=clamp, obs=np.full((K, len(times), n), PB.UNOBSERVED, dtype=np.uint8))
+    truth = np.concatenate([rng.integers(-1, 2, size=len(edges)), rng.integers(0, len(PB.TH_LO), size=n)]).astype(np.int8)
+    obs = np.asarray(O.simulate_fn(prob, truth), dtype=np.uint8).reshape(K, len(times), n).copy()
+    obs[:, :, rng.choice(n, size=n // 2, replace=False)] = PB.UNOBSERVED
+    prob.obs = obs
+    assert int((src == 0).sum()) == hub_out
+    return prob
+
+
+def test_hub_with_more_than_256_out_edges_on_the_static_kernel(B):
+    prob = hub_problem()
+    orc = O.Oracle(prob)
+    R, steps = 16, 1500
+    sched = PB.make_schedule(R, steps, n_levels=10)
+    hub_edges = np.nonzero(prob.edge_src == 0)[0]
+    with CHandle(B, prob, sched) as hd:
+        B.sa_set_trace(hd.h, list(range(R)), steps)
+        B.sa_run(hd.h, steps)
+        assert B.sa_get_info(hd.h)["variant"] == 4                        # N = 800: the static kernel
+        refs = oracle_chains(orc, sched, list(range(R)), steps)
+        # the case is only worth its name if non-zero hub edges are proposed while the hub has exactly 257 non-zero
+        # out-edges (= 1 mod 256, where "to 0" would be struck by mistake): replay the oracle's traces and count
+        is_hub = np.zeros(prob.n_params, dtype=bool)
+        is_hub[hub_edges] = True
+        hits = 0
+        for c, ref in enumerate(refs):
+            x = orc.init_chain(sched.seed, c, constrained=True)[0].copy()
+            tr = O.unpack_trace(ref["trace"])
+            count = int((x[is_hub] != 0).sum())
+            for p, code, acc, null in zip(tr["param"].tolist(), tr["code"].tolist(), tr["accepted"].tolist(), tr["null_move"].tolist()):
+                hits += int(is_hub[p] and x[p] != 0 and count == 257)
+                if acc and not null:
+                    new = code - 1 if p < prob.n_edges else code
+                    if is_hub[p]:
+                        count += int(new != 0) - int(x[p] != 0)
+                    x[p] = new
+            assert np.array_equal(x, ref["cur"])
+        assert hits >= 15, hits
+        check(B, hd, orc, list(range(R)), steps, B.sa_get_trace(hd.h, R, steps))
