@@ -86,8 +86,12 @@ typedef struct {
  * n_steps <= 127, n_obs <= 127, E < 2^24, state entries x words per entry x 4 <= 65535 bytes (about
  * 16 000 nodes at K <= 4, 4 000 at K <= 16).  On failure *out = NULL.
  * The host-side plans of a problem (tens of milliseconds) are kept, keyed by the problem's bytes, for the next
- * sa_create on the same problem (the last eight problems; thread safe). */
+ * sa_create on the same problem (the last eight problems, the oldest making room for a ninth; thread safe). */
 int sa_create(const sa_network *net, const sa_observations *obs, const sa_schedule *sched, sa_handle **out);
+
+/* Forget the kept host plans: the next sa_create on any problem plans from scratch (host only; what a
+ * measurement of the cold path calls between handles, bench.py's e2e.cold_plan).  Always SA_OK. */
+int sa_clear_plan_cache(void);
 
 /* Advance every chain by `steps` SA steps (Table 1 inner loop :130-149; SURVEY.md
  * §8(c)-3): propose, simulate all K conditions for T steps, score, accept/reject, commit.
@@ -254,7 +258,7 @@ typedef struct sap_handle sap_handle;            /* opaque, owned by the library
 
 typedef struct {
   int32_t n_nodes, n_edges;                      /* N <= 256, E */
-  const int32_t *edge_src, *edge_dst;            /* [E], no self-loops, no duplicate (src,dst) */
+  const int32_t *edge_src, *edge_dst;            /* [E], no duplicate (src,dst); src == dst (autoregulation) allowed */
   const uint8_t *fast;                           /* [N] 1 = speed range {10,11,12}, 0 = {1..6} */
 } sap_network;
 
@@ -275,8 +279,8 @@ typedef struct {
  * repair pass of DESIGN.md reading P6, Philox domain 2, so that every chain starts from a valid
  * vector) and evaluate it.  sched is the same structure as for sa_create; dmax should be
  * at least the largest objective (6 per measured entry) if no worse move is to be rejected outright.
- * Validation (SA_EINVAL): counts > 0, N <= 256, T <= 4095, endpoints in range, no self-loop / duplicate
- * edge, fast in {0,1}, states in {0,1,2}, ref in {0,1,2,255}, at most 256 edge slots per lane
+ * Validation (SA_EINVAL): counts > 0, N <= 256, T <= 4095, endpoints in range, no duplicate edge
+ * (a self-loop is an edge like any other here, unlike in the config model), fast in {0,1}, states in {0,1,2}, ref in {0,1,2,255}, at most 256 edge slots per lane
  * (in-degrees), and with SAP_CONSTRAINED an in-edge and an out-edge at every node. */
 int sap_create(const sap_network *net, const sap_observations *obs, const sa_schedule *sched, uint32_t flags,
                sap_handle **out);

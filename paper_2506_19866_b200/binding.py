@@ -20,7 +20,7 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_imma_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_level_sync_static", "sa_get_dense_info", "sa_get_level_stats",
+           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_level_sync_static", "sa_clear_plan_cache", "sa_get_dense_info", "sa_get_level_stats",
            "sap_create", "sap_run", "sap_run_levels", "sap_best", "sap_destroy", "sap_eval", "sap_simulate",
            "sap_get_chain", "sap_get_fitness", "sap_set_trace", "sap_get_trace", "sap_get_level_stats", "sap_get_info",
            "sap_set_stream", "sap_jit_check")
@@ -208,6 +208,10 @@ def sa_run(h: int, steps: int) -> None:
 
 def sa_run_levels(h: int, n_levels: int, group_size: int = 0) -> None:
     _check(_lib.sa_run_levels(h, n_levels, group_size), "sa_run_levels")
+
+
+def sa_clear_plan_cache() -> None:
+    _check(_lib.sa_clear_plan_cache(), "sa_clear_plan_cache")
 
 
 def sa_level_sync_static(h: int, group_size: int = 0) -> None:

@@ -1,6 +1,7 @@
 """Builds libternary_sa.so in-tree with nvcc for sm_100a (cross-compiles without a GPU).
 
     python -m paper_2506_19866_b200.build [--force] [--verbose]
+    python -m paper_2506_19866_b200.build --microbench      # only the stand-alone microbenchmarks, on request
 """
 from __future__ import annotations
 
@@ -64,7 +65,7 @@ MICRO_OUT = os.path.join(HERE, "build")
 
 def build_microbench(force: bool = False) -> None:
     """The stand-alone microbenchmarks behind the roofline (csrc/microbench/*.cu -> build/<name>, run by hand on a B200;
-    profiles/r2c_microbench.md has their output)."""
+    profiles/r2c_microbench.md has their output).  Never part of build(): the library must not depend on them."""
     os.makedirs(MICRO_OUT, exist_ok=True)
     for f in sorted(os.listdir(MICRO)):
         if not f.endswith(".cu"):
@@ -75,7 +76,6 @@ def build_microbench(force: bool = False) -> None:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    build_microbench(force)
     if not force and not stale():
         return LIB
     embed_static_source()
@@ -90,4 +90,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
+    if "--microbench" in sys.argv:
+        build_microbench(force="--force" in sys.argv)
+        print(MICRO_OUT)
+        sys.exit(0)
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))

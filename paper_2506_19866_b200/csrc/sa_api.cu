@@ -255,7 +255,9 @@ tsa::PlanOptions plan_options(int64_t n_chains, int sm_count) {
 // Host plans (edge schedule, bank classes, 2:4 row search, fragment tables) are a pure function of the problem and
 // the options, and take tens of milliseconds: sa_create keeps the last few, keyed by the problem's bytes, so that a
 // second handle on the same problem (another chain range, another schedule, a restart) only pays for the device side.
-struct CachedPlans { tsa::Plan plan; tsa::DensePlan dplan; };
+struct CachedPlans { tsa::Plan plan; tsa::DensePlan dplan; uint64_t born = 0; };
+constexpr size_t kCachedPlans = 8;
+uint64_t g_plans_clock = 0;
 std::mutex g_plans_mu;
 std::map<std::string, std::shared_ptr<const CachedPlans>> g_plans;
 
@@ -301,6 +303,12 @@ int sa_geometric_table(double t0, double t_end, int32_t L, int32_t D, uint32_t* 
   return SA_OK;
 }
 
+int sa_clear_plan_cache(void) {
+  std::lock_guard<std::mutex> lock(g_plans_mu);
+  g_plans.clear();
+  return SA_OK;
+}
+
 int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedule* sched, sa_handle** out) {
   if (!out) return set_err(SA_EINVAL, "out is NULL");
   *out = nullptr;
@@ -336,7 +344,13 @@ int sa_create(const sa_network* net, const sa_observations* obs, const sa_schedu
         auto entry = std::make_shared<CachedPlans>();
         entry->plan = h->plan; entry->dplan = h->dplan;
         std::lock_guard<std::mutex> lock(g_plans_mu);
-        if (g_plans.size() >= 8) g_plans.clear();
+        if (g_plans.size() >= kCachedPlans && !g_plans.count(key)) {          // full: the oldest entry makes room
+          auto oldest = g_plans.begin();
+          for (auto it = g_plans.begin(); it != g_plans.end(); ++it)
+            if (it->second->born < oldest->second->born) oldest = it;
+          g_plans.erase(oldest);
+        }
+        entry->born = ++g_plans_clock;
         g_plans[key] = entry;
       }
     }
@@ -690,6 +704,11 @@ int sa_set_trace(sa_handle* h, const int32_t* chains, int32_t n, int64_t max_ste
   const int32_t* d_row = nullptr;
   int rc = h->trace_pool.upload(row, &d_row, h->stream);
   if (rc) return rc;
+  // n * max_steps records of 8 bytes: refuse what cannot be a device buffer before the product can wrap
+  if (max_steps > tsa::kMaxTraceRecords || (int64_t)n * max_steps > tsa::kMaxTraceRecords) {
+    h->trace_pool.clear();
+    return set_err(SA_EINVAL, "sa_set_trace: more than 2^34 trace records (128 GiB) asked for");
+  }
   const size_t bytes = (size_t)n * (size_t)max_steps * 8;
   uint64_t* rec = (uint64_t*)h->trace_pool.alloc(bytes, h->stream);
   if (!rec) { h->trace_pool.clear(); return set_err(SA_ENOMEM, "device allocation failed (trace)"); }

@@ -11,6 +11,8 @@
 
 namespace tsa {
 
+constexpr int64_t kMaxTraceRecords = (int64_t)1 << 34;   // *_set_trace: chains x steps, 8 bytes each
+
 inline thread_local std::string g_err;
 inline sa_alloc_fn g_alloc = nullptr;
 inline sa_free_fn g_free = nullptr;

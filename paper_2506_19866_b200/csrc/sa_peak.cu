@@ -83,7 +83,12 @@ extern "C" int sa_int32_peak(double out[6]) {
     return SA_ECUDA;
   uint32_t* sink = nullptr;
   unsigned long long* clk = nullptr;
-  if (cudaMalloc(&sink, 16) != cudaSuccess || cudaMalloc(&clk, 16) != cudaSuccess) return SA_ENOMEM;
+  if (cudaMalloc(&sink, 16) != cudaSuccess || cudaMalloc(&clk, 16) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(sink);                                      // NULL if the first allocation is the one that failed
+    cudaFree(clk);
+    return SA_ENOMEM;
+  }
   const int trips = 4096;
   double hz = 0.0;
   cudaError_t e = run_one<0>(sms, trips, sink, clk, &out[0], nullptr);
@@ -176,7 +181,12 @@ extern "C" int sa_imma_peak(double out[4]) {
     return SA_ECUDA;
   int* sink = nullptr;
   unsigned long long* clk = nullptr;
-  if (cudaMalloc(&sink, 16) != cudaSuccess || cudaMalloc(&clk, 16) != cudaSuccess) return SA_ENOMEM;
+  if (cudaMalloc(&sink, 16) != cudaSuccess || cudaMalloc(&clk, 16) != cudaSuccess) {
+    cudaGetLastError();
+    cudaFree(sink);                                      // NULL if the first allocation is the one that failed
+    cudaFree(clk);
+    return SA_ENOMEM;
+  }
   double hz = 0.0;
   cudaError_t e = run_imma<false>(sms, 8192, sink, clk, &out[0], nullptr);
   if (e == cudaSuccess) e = run_imma<true>(sms, 8192, sink, clk, &out[1], &hz);

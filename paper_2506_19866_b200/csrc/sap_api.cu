@@ -306,6 +306,11 @@ int sap_set_trace(sap_handle* h, const int32_t* chains, int32_t n, int64_t max_s
   const int32_t* d_row = nullptr;
   int rc = h->trace_pool.upload(row, &d_row, h->stream);
   if (rc) return rc;
+  // n * max_steps records of 8 bytes: refuse what cannot be a device buffer before the product can wrap
+  if (max_steps > tsa::kMaxTraceRecords || (int64_t)n * max_steps > tsa::kMaxTraceRecords) {
+    h->trace_pool.clear();
+    return set_err(SA_EINVAL, "sap_set_trace: more than 2^34 trace records (128 GiB) asked for");
+  }
   const size_t bytes = (size_t)n * (size_t)max_steps * 8;
   unsigned long long* rec = (unsigned long long*)h->trace_pool.alloc(bytes, h->stream);
   if (!rec) { h->trace_pool.clear(); return set_err(SA_ENOMEM, "device allocation failed (trace)"); }

@@ -28,7 +28,7 @@ int build_paper_plan(const sap_network* net, const sap_observations* obs, bool n
   for (int e = 0; e < E; ++e) {
     const int s = pl.src[e], d = pl.dst[e];
     if (s < 0 || s >= N || d < 0 || d >= N) return fail("edge endpoint out of range");
-    if (s == d) return fail("self-loop");
+    // s == d is allowed: autoregulation is an edge like any other in PAPER.md:55-70, and the oracle takes it too
     if (!seen.insert({s, d}).second) return fail("duplicate edge");
   }
   pl.fast.assign(net->fast, net->fast + N);

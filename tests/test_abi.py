@@ -171,10 +171,10 @@ def test_sap_create_validation(B, paper_hpg):
             B.sap_create(prob, sc, flags)
         assert ei.value.code == B.SA_EINVAL and match in str(ei.value), str(ei.value)
 
-    p = copy.copy(good); p.edge_src = good.edge_src.copy(); p.edge_src[0] = p.edge_dst[0]
-    bad(p, sched, "self-loop")
     p = copy.copy(good); p.edge_src = good.edge_src.copy(); p.edge_dst = good.edge_dst.copy()
     p.edge_src[1], p.edge_dst[1] = p.edge_src[0], p.edge_dst[0]
+    bad(p, sched, "duplicate")
+    p.edge_dst[0] = p.edge_src[0]; p.edge_dst[1] = p.edge_src[1]          # the same self-loop twice; one alone is allowed
     bad(p, sched, "duplicate")
     p = copy.copy(good); p.edge_dst = good.edge_dst.copy(); p.edge_dst[0] = good.n_nodes
     bad(p, sched, "out of range")

@@ -390,3 +390,57 @@ def test_paper_mtb_hundred_thousand_chains(B, paper_problems):
         assert B.sap_get_info(hd.h)["lanes_per_chain"] == 16
         B.sap_run(hd.h, 20)
         check_chains(B, hd, orc, list(range(0, R, 7)) + [R - 1], 20)
+
+
+# ------------------------------------------------------------------------------------- autoregulation
+def with_self_loops(prob, count=6):
+    """A copy of the problem in which `count` edges are turned into self-loops (src -> src).  Only edges whose target
+    keeps at least two other in-edges are taken, so that every node still has an in-edge and an out-edge."""
+    src, dst = prob.edge_src.copy(), prob.edge_dst.copy()
+    have = set(zip(src.tolist(), dst.tolist()))
+    indeg = np.bincount(dst, minlength=prob.n_nodes)
+    done = 0
+    for e in range(prob.n_edges):
+        s, d = int(src[e]), int(dst[e])
+        if done < count and indeg[d] >= 3 and (s, s) not in have:
+            have.discard((s, d)); have.add((s, s))
+            indeg[d] -= 1; indeg[s] += 1
+            dst[e] = s
+            done += 1
+    assert done == count
+    out = copy.copy(prob)
+    out.edge_src, out.edge_dst = src, dst
+    return out
+
+
+@pytest.mark.parametrize("name,R,flags", [("paper_hpg", 64, 0), ("paper_hpg", 64, 1), ("paper_mtb", 48, 1), ("paper_mtb", 9600, 1)])
+def test_self_loops_are_edges_like_any_other(B, paper_problems, name, R, flags):
+    prob = with_self_loops(paper_problems(name))
+    assert int((prob.edge_src == prob.edge_dst).sum()) == 6
+    orc = OP.PaperOracle(prob)
+    sched = PB.paper_schedule(R, 10, 80, prob.max_objective)
+    chains = PB.spread_chains(R, 24)
+    with Handle(B, prob, sched, flags) as hd:
+        B.sap_set_trace(hd.h, chains, 800)
+        B.sap_run(hd.h, 800)
+        tr = B.sap_get_trace(hd.h, len(chains), 800)
+        check_chains(B, hd, orc, chains, 800, tr)
+        loops = np.nonzero(prob.edge_src == prob.edge_dst)[0]
+        param = OP.unpack_trace(tr)["param"]                             # weight, polarity and threshold of edge e: e, E + e, 2E + e
+        assert np.isin(param[param < 3 * prob.n_edges] % prob.n_edges, loops).any(), "no self-loop parameter was ever proposed"
+        x = PB.random_paper_params(prob, 64, 5)
+        assert np.array_equal(B.sap_eval(hd.h, x), orc.objective_batch(x))
+        assert np.array_equal(B.sap_simulate(prob, x[0]), orc.simulate(x[0]))
+
+
+def test_set_trace_refuses_sizes_that_cannot_be_a_buffer(B, paper_problems):
+    prob = paper_problems("paper_tiny")
+    sched = PB.paper_schedule(8, 4, 25, prob.max_objective)
+    with Handle(B, prob, sched) as hd:
+        for n, steps in ((2, 2 ** 62), (8, 2 ** 61), (1, 2 ** 34 + 1)):
+            with pytest.raises(B.SaError) as err:
+                B.sap_set_trace(hd.h, list(range(n)), steps)
+            assert err.value.code == B.SA_EINVAL and "trace records" in str(err.value)
+        B.sap_set_trace(hd.h, [5], 40)
+        B.sap_run(hd.h, 40)
+        check_chains(B, hd, OP.PaperOracle(prob), [5], 40, B.sap_get_trace(hd.h, 1, 40))

@@ -476,3 +476,20 @@ def test_int32_peak_microbenchmark_runs(B):
         # never above one instruction per scheduler per clock, never absurdly low
         ceiling = pk["sm_count"] * 4 * pk["sm_hz"]
         assert 0.05 * ceiling < pk[k] < 1.05 * ceiling, (k, pk)
+
+
+@pytest.mark.gpu
+def test_set_trace_refuses_sizes_that_cannot_be_a_buffer(B, problems_cache):
+    """chains x steps x 8 bytes is checked before it can wrap or reach the allocator (2^34 records at most)."""
+    prob = problems_cache("tiny")
+    sched = PB.default_schedule("tiny")
+    with Handle(B, prob, sched) as hd:
+        for n, steps in ((2, 2 ** 62), (8, 2 ** 61), (1, 2 ** 34 + 1), (8, 2 ** 32)):
+            with pytest.raises(B.SaError) as err:
+                B.sa_set_trace(hd.h, list(range(n)), steps)
+            assert err.value.code == B.SA_EINVAL and "trace records" in str(err.value)
+        B.sa_set_trace(hd.h, [0, 3], 50)                                  # and tracing still works afterwards
+        B.sa_run(hd.h, 50)
+        tr = B.sa_get_trace(hd.h, 2, 50)
+        ref = O.Oracle(prob).run_chain(sched, 3, 50)
+        assert np.array_equal(tr[1], ref["trace"])
