@@ -30,6 +30,7 @@ sys.path.insert(0, ROOT)
 
 import numpy as np  # noqa: E402
 
+from paper_2506_19866_b200 import inst_counts as IC  # noqa: E402
 from paper_2506_19866_b200 import problems as PB  # noqa: E402
 
 METRIC = "sa_chain_steps_per_sec"
@@ -37,7 +38,6 @@ UNIT = "chain-steps/s"
 WORKLOADS = sorted(PB.CONFIGS) + ["paper_hpg", "paper_mtb"]
 # warp-instructions one chain-step executes, per kernel, from the committed ncu captures (smsp__inst_executed.sum
 # of one launch / its chain-steps); bench.py multiplies them by the chain-steps/s it measures live
-INST_COUNTS = os.path.join(ROOT, "profiles", "inst_counts.json")
 
 
 def _measured_peaks():
@@ -49,11 +49,7 @@ def _measured_peaks():
 
 
 def _inst_counts():
-    try:
-        with open(INST_COUNTS) as f:
-            return json.load(f)
-    except Exception:
-        return {}
+    return IC.load()
 
 
 def cpu_model() -> str:
@@ -324,7 +320,11 @@ def run_ours(args) -> dict:
              "traffic": None,
              "alg_ops_per_chain_step": prob.alg_ops_per_step,
              "useful_frac": prob.alg_ops_per_step * rate / (issue_peak * 32)}
-        if cnt.get("kernel") == kn and cnt.get("warp_inst_per_chain_step"):
+        # a count only applies to the kernel text and launch geometry it was captured on (inst_counts.py)
+        family = IC.KERNELS.get(kn, (None,))[0]
+        stale = (IC.stale_reason(cnt, kn, B.sa_kernel_source_id(family), chains, m["info"].get("launch") or m["info"]["paper"]) if family
+                 else f"no instruction count for kernel {kn} on workload {name} in profiles/inst_counts.json")
+        if stale is None:
             r["warp_inst_per_chain_step"] = cnt["warp_inst_per_chain_step"]
             r["warp_inst_source"] = cnt.get("source")
             r["achieved"] = cnt["warp_inst_per_chain_step"] * rate / 1e12
@@ -338,7 +338,7 @@ def run_ours(args) -> dict:
         else:
             r["achieved"] = None
             r["frac"] = None
-            r["frac_note"] = f"no instruction count for kernel {kn} on workload {name} in profiles/inst_counts.json"
+            r["frac_note"] = stale
         if not is_paper(name) and m["info"]["launch"]["variant"] == 5 and imma:
             # second ceiling of the dense kernel: MMA instructions per time step against the rate of the
             # legacy tensor path measured in this run (sa_imma_peak)

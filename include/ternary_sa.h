@@ -227,6 +227,13 @@ int sa_get_dense_info(sa_handle *h, int64_t info[8]);
 #define SA_KERNEL_DENSE   3
 int sa_select_kernel(sa_handle *h, int family);
 
+/* Host only: a 64-bit FNV-1a of the run-time compiled source text this library carries for one kernel family
+ * (SA_KERNEL_STATIC, SA_KERNEL_DENSE, or SA_KERNEL_PAPER for the sap_* kernels).  profiles/inst_counts.json stores it
+ * beside every instruction count taken with ncu; bench.py reports no issue-slot fraction when the loaded library's
+ * differs (the count belongs to another kernel text), and a CPU test compares both with the sources in the tree. */
+#define SA_KERNEL_PAPER   4
+int sa_kernel_source_id(int32_t family, uint64_t *id);
+
 /* Host only (no GPU needed): build the plan of a problem for n_chains chains and compile the
  * statically scheduled kernel for it.  info[0] = 1 if the static kernel applies, [1] = warps per
  * chain, [2] = tiers, [3] = edge slots per thread, [4] = cubin bytes, [5] = shared memory bytes per

@@ -20,12 +20,12 @@ SA_OK, SA_EINVAL, SA_ENOMEM, SA_ECUDA = 0, -1, -2, -3
 EXPORTS = ("sa_create", "sa_run", "sa_best", "sa_destroy", "sa_eval", "sa_simulate", "sa_get_chain",
            "sa_get_fitness", "sa_set_trace", "sa_get_trace", "sa_geometric_table", "sa_get_info",
            "sa_set_stream", "sa_set_allocator", "sa_int32_peak", "sa_imma_peak", "sa_last_error", "sa_plan_info",
-           "sa_select_kernel", "sa_jit_check", "sa_run_levels", "sa_level_sync_static", "sa_clear_plan_cache", "sa_get_dense_info", "sa_get_level_stats",
+           "sa_select_kernel", "sa_kernel_source_id", "sa_jit_check", "sa_run_levels", "sa_level_sync_static", "sa_clear_plan_cache", "sa_get_dense_info", "sa_get_level_stats",
            "sap_create", "sap_run", "sap_run_levels", "sap_best", "sap_destroy", "sap_eval", "sap_simulate",
            "sap_get_chain", "sap_get_fitness", "sap_set_trace", "sap_get_trace", "sap_get_level_stats", "sap_get_info",
            "sap_set_stream", "sap_jit_check")
 SAP_CONSTRAINED, SAP_LEVEL_STATS = 1, 2
-SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE = 0, 1, 2, 3
+SA_KERNEL_AUTO, SA_KERNEL_GENERIC, SA_KERNEL_STATIC, SA_KERNEL_DENSE, SA_KERNEL_PAPER = 0, 1, 2, 3, 4
 SA_CONSTRAINED, SA_LEVEL_STATS = 1, 2
 SA_LEVEL_SYNC_STATIC_MAX_GROUPS = 65536
 
@@ -307,6 +307,13 @@ def sa_plan_info(prob) -> dict:
 
 def sa_select_kernel(h: int, family: int) -> None:
     _check(_lib.sa_select_kernel(h, family), "sa_select_kernel")
+
+
+def sa_kernel_source_id(family: int) -> str:
+    """FNV-1a-64 (16 hex digits) of the run-time compiled source text the loaded library carries for a kernel family."""
+    out = C.c_uint64()
+    _check(_lib.sa_kernel_source_id(family, C.byref(out)), "sa_kernel_source_id")
+    return f"{out.value:016x}"
 
 
 def sa_jit_check(prob, n_chains: int) -> dict:

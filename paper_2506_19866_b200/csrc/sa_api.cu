@@ -787,6 +787,12 @@ int sa_jit_check(const sa_network* net, const sa_observations* obs, int32_t n_ch
   return SA_OK;
 }
 
+int sa_kernel_source_id(int32_t family, uint64_t* id) {
+  if (!id) return set_err(SA_EINVAL, "id is NULL");
+  if (!tsa::kernel_source_id(family, id)) return set_err(SA_EINVAL, "family must be SA_KERNEL_STATIC, SA_KERNEL_DENSE or SA_KERNEL_PAPER");
+  return SA_OK;
+}
+
 int sa_plan_info(const sa_network* net, const sa_observations* obs, int64_t info[16]) {
   if (!net || !obs || !info) return set_err(SA_EINVAL, "null argument");
   tsa::Plan pl;

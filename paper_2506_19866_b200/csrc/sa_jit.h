@@ -81,4 +81,8 @@ bool paper_kernel_compile(const std::vector<std::string>& defines, std::string* 
 const PaperKernels* paper_kernels_get(const PaperPlan& plan, std::string* why);
 int paper_kernel_launch(const StaticKernel* k, unsigned grid, void* stream, const tsa_paper::Params& params, std::string* why);
 
+// FNV-1a-64 of the NVRTC source text this library was built with: which = 2 statically scheduled kernel, 3 dense
+// kernel, 4 paper-model kernels.  false for any other value.
+bool kernel_source_id(int which, uint64_t* id);
+
 }  // namespace tsa

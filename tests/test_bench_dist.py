@@ -6,6 +6,7 @@ import subprocess
 import sys
 
 import numpy as np
+import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -106,3 +107,31 @@ def test_instruction_counts_file_names_existing_captures():
         assert c["warp_inst_per_chain_step"] > 0 and c["kernel"]
         cited = c["source"].split()[0]
         assert os.path.exists(os.path.join(ROOT, cited)), cited
+
+
+def test_instruction_counts_belong_to_the_kernels_in_the_tree():
+    """Every entry of profiles/inst_counts.json records the source text and the launch geometry it was captured on.
+    A kernel source changed without a fresh capture fails here (and bench.py would report `frac: null`)."""
+    from paper_2506_19866_b200 import build, inst_counts as IC
+    build.build()
+    from paper_2506_19866_b200 import binding as B
+    counts = IC.load()
+    for name in ("mtb", "hpg", "large", "paper_mtb", "paper_hpg"):
+        c = counts[name]
+        family, _ = IC.KERNELS[c["kernel"]]
+        tree, lib = IC.tree_source_id(c["kernel"]), B.sa_kernel_source_id(family)
+        assert lib == tree, f"libternary_sa.so carries another {c['kernel']} source than the tree: rebuild"
+        assert c.get("source_id") == tree, (f"{name}: the instruction count was captured on kernel source {c.get('source_id')}, the tree has "
+                                            f"{tree}: re-capture (python -m paper_2506_19866_b200.inst_counts update ...)")
+        assert c["geometry"]["chains"] > 0 and c["geometry"]["threads_per_cta"] > 0
+    # the check bench.py makes, on made-up handles
+    c = counts["mtb"]
+    launch = {k: v for k, v in c["geometry"].items() if k != "chains"}
+    lib = B.sa_kernel_source_id(B.SA_KERNEL_DENSE)
+    assert IC.stale_reason(c, "tsa_run_dense", lib, c["geometry"]["chains"], launch) is None
+    assert "geometry" in IC.stale_reason(c, "tsa_run_dense", lib, c["geometry"]["chains"], dict(launch, chains_per_cta=16))
+    assert "geometry" in IC.stale_reason(c, "tsa_run_dense", lib, 1024, launch)
+    assert "source" in IC.stale_reason(c, "tsa_run_dense", "0" * 16, c["geometry"]["chains"], launch)
+    assert "kernel" in IC.stale_reason(c, "tsa_run_static", lib, c["geometry"]["chains"], launch)
+    with pytest.raises(B.SaError):
+        B.sa_kernel_source_id(1)
