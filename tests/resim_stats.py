@@ -1,5 +1,5 @@
 """Does exact incremental re-simulation pay?  (north_star: "re-simulates only the conditions reachable
-from the mutated edge's target where that pays off"; VERDICT r1 missing #3-ii.)
+from the mutated edge's target where that pays off".)
 
 TEST / MEASUREMENT INFRASTRUCTURE: calls only oracle/ (and the shared input generators).  For SA
 chains of the config model it replays every step's candidate next to the current vector and counts,
@@ -16,7 +16,7 @@ current trajectory:
   * "no effect": the candidate's whole trajectory equals the current one (fitness unchanged);
   * "first divergence": the first t at which any condition differs.
 
-    python -m oracle.resim_stats [--chains 3] [--steps 600]
+    python tests/resim_stats.py [--chains 3] [--steps 600]
 
 prints one markdown table row per workload (the numbers quoted in DESIGN.md §11).
 """

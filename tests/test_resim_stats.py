@@ -1,8 +1,8 @@
-"""oracle/resim_stats.py (the measurement behind "incremental re-simulation: does it pay?")."""
+"""tests/resim_stats.py (the measurement behind "incremental re-simulation: does it pay?")."""
 import numpy as np
 
 from oracle import oracle as O
-from oracle import resim_stats as RS
+import resim_stats as RS
 from paper_2506_19866_b200 import problems as PB
 
 
